@@ -1,0 +1,103 @@
+/*
+ * phx_oracle.h -- C ABI of the CPU ORACLE for the PHOENIX RK4 hot path.
+ *
+ * TEST INFRASTRUCTURE, NOT PRODUCT.  Only tests/, __graft_entry__.smoke() and bench.py's
+ * cpu_baseline / --impl reference leg may load this library.  It shares no code with the CUDA
+ * path under paper_2411_18341_b200/ and neither side includes or imports the other.
+ *
+ * The oracle follows /root/reference/PAPER.md step by step, in the paper's own unfused form
+ * (separate K1..K4 buffers and a stage buffer, PAPER.md:100-144 Listing 1, :181 "six buffers"):
+ *   - Eq. (1)  PAPER.md:25      damped nonlinear Schroedinger equation
+ *   - Eqs. (2)-(6) PAPER.md:53-62  fixed-step RK4
+ *   - Eq. (8)  PAPER.md:203     five-point Laplacian with separate dx, dy
+ *   - Eqs. (16)-(17) PAPER.md:361-364  spinor, reservoir, TE-TM, coherent drive E, noise dW
+ *   - Eq. (22) PAPER.md:454-456  complex Wiener noise covariance
+ * All arithmetic is IEEE double, one thread, no FMA contraction, no blocking or fusion.
+ * The readings taken where the paper is silent or garbled are listed in DESIGN.md section 3.
+ *
+ * Pins (tests/test_oracle_*.py, all -m "not gpu"): stencil vs. dense brute force and vs. its
+ * Fourier symbol; plane-wave amplification R(z)^N; loss and norm closed forms; reduction of
+ * plane-wave states to a 0-dimensional RK4 written independently in Python (nonlinearity,
+ * reservoir, spinor, TE-TM, drive); reservoir-only closed form; sine eigenmodes for zero
+ * boundaries; RK4 order test; Philox4x32-10 known-answer vectors; normal-map moments.
+ * Parity unpinned: statistics of full noisy trajectories beyond the integer stream, the
+ * normal map's moments and short segments (the dynamics are chaotic).
+ */
+#ifndef PHX_ORACLE_H
+#define PHX_ORACLE_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* Physical parameters, as in Eqs. (1), (16), (17), (22). */
+typedef struct {
+    double hbar, m;          /* Eq. (1) */
+    double g;                /* same-spin nonlinearity g |psi_s|^2 */
+    double g_x;              /* cross-spin nonlinearity g_x |psi_-s|^2, Eq. (16) */
+    double g_r;              /* reservoir interaction g_r n, Eq. (16) */
+    double R;                /* condensation rate, Eqs. (16), (17) */
+    double gamma_c;          /* loss gamma of psi, Eq. (1) / (16) */
+    double gamma_r;          /* reservoir loss, Eq. (17) */
+    double beta;             /* Delta_LT of J = Delta_LT (d_x -+ i d_y)^2 */
+    double dt;               /* RK4 step */
+    double noise_scale;      /* nu, scales the Wiener noise variance */
+    double density_offset;   /* 1/DeltaV of the renormalised density, PAPER.md:452 (0 = off) */
+    double omega;            /* drive frequency: E(r,t) = E(r) exp(-i omega t) */
+} orc_params;
+
+/* Canonical derived coefficients ("step 0").  Each is evaluated in
+ * double with exactly the expression in orc_derive_coeffs and then, when prec32 != 0,
+ * rounded once to float and widened back. */
+enum {
+    ORC_CX = 0, ORC_CY, ORC_IH, ORC_G, ORC_GX, ORC_GR, ORC_RR, ORC_HGC, ORC_GAMR,
+    ORC_BXX, ORC_BYY, ORC_BXY, ORC_DT, ORC_DT6, ORC_DT3, ORC_SIG2, ORC_DOFF, ORC_OMEGA,
+    ORC_NCOEF
+};
+
+typedef struct {
+    int32_t nx, ny, batch;       /* arrays are [batch][ny][nx], x fastest */
+    int32_t spinor;              /* 0: psi_+ only; 1: psi_+ and psi_- */
+    int32_t reservoir;           /* 0: n == 0;     1: n_+ (and n_- if spinor) integrated */
+    int32_t noise;               /* 0/1: add dW after each step (Eq. 22) */
+    int32_t bc_x, bc_y;          /* 0 periodic, 1 zero */
+    uint32_t seed;               /* Philox key word 0 */
+    double coef[ORC_NCOEF];
+    const double* V;             /* [ny][nx] real, shared by the batch; NULL = 0 */
+    const double* P;             /* [ny][nx] real pump P_+ = P_-; NULL = 0 */
+    const double* E;             /* [ny][nx] complex drive amplitude E_+ = E_-; NULL = 0 */
+} orc_problem;
+
+void orc_derive_coeffs(const orc_params* p, double dx, double dy, int32_t prec32,
+                       double out[ORC_NCOEF]);
+
+/* One evaluation of the derivative f (the paper's CALCULATE_K) on ONE batch element at time t.
+ * psi_* are interleaved complex [ny][nx]; n_* real.  Unused fields may be NULL. */
+void orc_derivative(const orc_problem* pb, double t,
+                    const double* psi_p, const double* psi_m, const double* n_p, const double* n_m,
+                    double* K_p, double* K_m, double* Kn_p, double* Kn_m);
+
+/* n_steps RK4 steps in place on all batch elements; step0 = number of steps already completed
+ * (keys the noise and fixes t = step0*dt for the drive).  Returns 0, or 1 on bad arguments. */
+int32_t orc_step_rk4(const orc_problem* pb, double* psi_p, double* psi_m, double* n_p, double* n_m,
+                     uint64_t step0, int64_t n_steps);
+
+/* Philox4x32-10 (Salmon et al., SC'11): one block. */
+void orc_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]);
+
+/* The four 32-bit words drawn for every (realisation, cell) at step `step`:
+ * out[batch][ny][nx][4] = Philox(ctr=(cell, step_lo, step_hi, 0), key=(seed, realisation)). */
+void orc_noise_u32(int32_t nx, int32_t ny, int32_t batch, uint32_t seed, uint64_t step, uint32_t* out);
+
+/* Map two words to a standard complex normal pair (xi1, xi2) by Box-Muller. */
+void orc_normal_pair(uint32_t w0, uint32_t w1, double* xi1, double* xi2);
+
+/* <|psi|^2>(x,y) = (1/batch) sum_r |psi_r|^2 ; psi interleaved complex [batch][ny][nx]. */
+void orc_ensemble_mean_density(int32_t nx, int32_t ny, int32_t batch, const double* psi, double* out);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,164 @@
+/*
+ * phx.h -- C ABI of libphx: B200-native (sm_100a) fixed-step RK4 time stepping of the damped 2D
+ * nonlinear Schroedinger / Gross-Pitaevskii equation and its integrated extensions
+ * (PHOENIX, arXiv 2411.18341; citations are /root/reference/PAPER.md:<line>).
+ *
+ * What the library computes (DESIGN.md section 2 gives the discrete formulas):
+ *   Eq. (1)   PAPER.md:25       i hbar d_t psi = (-hbar^2/2m lap + V + g|psi|^2 - i hbar gamma/2) psi
+ *   Eq. (8)   PAPER.md:203      lap = five-point stencil with separate dx, dy
+ *   Eqs. (2)-(6) PAPER.md:53-62 fixed-step RK4 (weights of Listing 1)
+ *   Eq. (16)  PAPER.md:361      spinor psi_+-, g_x |psi_-+|^2, g_r n, (i hbar/2)(R n - gamma),
+ *                               TE-TM coupling J_+- = Delta_LT (d_x -+ i d_y)^2 on psi_-+,
+ *                               coherent drive E exp(-i omega t), Wiener noise dW
+ *   Eq. (17)  PAPER.md:364      d_t n = P - (gamma_r + R |psi|^2) n
+ *   Eq. (22)  PAPER.md:454-456  <dW dW*> = (R n + gamma_c)/(2 DeltaV), <dW dW> = 0
+ *   boundaries PAPER.md:369     periodic or zero, independently in x and y
+ *
+ * Conventions
+ *   - Every call returns a phx_status; 0 = success, >= 100 = warning (state still valid).
+ *     No exception or abort crosses this boundary.  Arguments are validated before device work.
+ *   - Arrays are row-major [batch][ny][nx], x fastest.  A complex field is interleaved (re, im) of
+ *     the working real type T (float for PHX_C32, double for PHX_C64); reservoirs, V and P are real T.
+ *   - phx_mem says where a caller pointer lives: PHX_HOST (pageable or pinned) or PHX_DEVICE.
+ *   - OWNERSHIP: the caller owns all device memory -- the workspace and every PHX_DEVICE source or
+ *     destination -- and the stream.  The library allocates no device memory: state fields, stage
+ *     buffers, accumulators, V, P, E and the step counter all live in the workspace.  The handle is
+ *     host memory owned by the library until phx_destroy_grid.
+ *   - One handle is used by one thread at a time; handles are independent.
+ *   - phx_step_rk4 is asynchronous on the stream.  A CUDA failure is reported by the next
+ *     synchronising call (phx_read_field, phx_sync, ...) and is sticky (PHX_ERR_CUDA).
+ *   - The step counter is part of the state: k calls of one step == one call of k steps, bit for
+ *     bit (it keys the noise and fixes the drive phase t = step*dt).
+ *   - There is no CPU fallback: without a CUDA device phx_create_grid fails with PHX_ERR_CUDA.
+ */
+#ifndef PHX_H
+#define PHX_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct phx_grid phx_grid; /* opaque */
+
+typedef enum {
+    PHX_OK = 0,
+    PHX_ERR_INVALID_ARG = 1,   /* NULL pointer, size < 3, non-positive dx/dy/dt, zero hbar or m, bad enum */
+    PHX_ERR_BAD_STATE = 2,     /* e.g. stepping before phx_set_params */
+    PHX_ERR_UNSUPPORTED = 3,   /* field not present in the model, variant not available for this grid */
+    PHX_ERR_CUDA = 4,          /* CUDA runtime failure (sticky); see phx_last_error */
+    PHX_ERR_WORKSPACE = 5,     /* workspace NULL, misaligned (256 B) or smaller than phx_workspace_bytes */
+    PHX_WARN_UNSTABLE = 100    /* (hbar/2m)(4/dx^2+4/dy^2) dt exceeds the RK4 limit 2.78; parameters were set */
+} phx_status;
+
+typedef enum { PHX_C32 = 0, PHX_C64 = 1 } phx_precision;
+typedef enum { PHX_SCALAR = 0, PHX_RESERVOIR = 1, PHX_SPINOR = 2, PHX_SPINOR_RESERVOIR = 3 } phx_model;
+typedef enum { PHX_HOST = 0, PHX_DEVICE = 1 } phx_mem;
+typedef enum { PHX_PSI = 0, PHX_PSI_MINUS = 1, PHX_N = 2, PHX_N_MINUS = 3 } phx_field;
+typedef enum { PHX_BC_PERIODIC = 0, PHX_BC_ZERO = 1 } phx_boundary;
+
+/* Kernel variants (all compute the same RK4 step; they differ in how often data crosses HBM). */
+typedef enum {
+    PHX_VARIANT_AUTO = 0,
+    PHX_VARIANT_STAGE = 1,     /* one fused kernel per RK stage (4 launches per step) */
+    PHX_VARIANT_STEP = 3,      /* one kernel per RK4 step, four stages on a haloed tile in shared memory */
+    PHX_VARIANT_RESIDENT = 4   /* whole grid resident on chip, many steps per launch (small grids) */
+} phx_variant;
+
+typedef struct {
+    int32_t nx, ny;            /* cells in x and y, each >= 3 */
+    int32_t batch;             /* independent realisations sharing V, P, E (>= 1) */
+    double dx, dy;             /* cell sizes (> 0) */
+    int32_t prec;              /* phx_precision */
+    int32_t model;             /* phx_model */
+    int32_t noise;             /* 0/1: add the Wiener increment of Eq. (22) after every step */
+    int32_t bc_x, bc_y;        /* phx_boundary per axis */
+    void* workspace;           /* DEVICE memory owned by the caller, 256-byte aligned */
+    size_t workspace_bytes;    /* >= phx_workspace_bytes(desc) */
+    void* stream;              /* cudaStream_t owned by the caller; NULL = legacy default stream */
+} phx_grid_desc;
+
+typedef struct {
+    double hbar, m;            /* Eq. (1); both non-zero */
+    double g;                  /* same-spin nonlinearity */
+    double g_x;                /* cross-spin nonlinearity (spinor models) */
+    double g_r;                /* reservoir interaction (reservoir models) */
+    double R;                  /* condensation rate */
+    double gamma_c;            /* loss of psi (gamma of Eq. (1)) */
+    double gamma_r;            /* reservoir loss */
+    double beta;               /* Delta_LT of the TE-TM coupling (spinor models) */
+    double dt;                 /* RK4 step (> 0) */
+    double noise_scale;        /* nu: multiplies the noise variance (1 = Eq. (22) as printed) */
+    double density_offset;     /* 1/DeltaV subtracted from |psi|^2; 0 = off */
+    double omega;              /* drive frequency, E(r,t) = E(r) exp(-i omega t) */
+    uint32_t seed;             /* Philox key word 0 (word 1 is the realisation index) */
+} phx_params;
+
+/* Number of canonical coefficients returned by phx_get_coeffs, in the order
+ * cx cy ih g gx gr Rr hgc gamr bxx byy bxy dt dt6 dt3 sig2 doff omega. */
+#define PHX_NCOEF 18
+
+/* Bytes of device workspace phx_create_grid needs for this descriptor (workspace fields ignored).
+ * Returns 0 if the descriptor is invalid. */
+size_t phx_workspace_bytes(const phx_grid_desc* desc);
+
+/* Creates a handle.  All state fields, V, P and E start as zero; the step counter starts at 0.
+ * Errors: INVALID_ARG, WORKSPACE, CUDA (no device / not sm_100). *out is NULL on error. */
+phx_status phx_create_grid(phx_grid** out, const phx_grid_desc* desc);
+
+/* Sets the physical parameters and derives the canonical coefficient set (rounded once to T).
+ * May return PHX_WARN_UNSTABLE (parameters are set nevertheless). */
+phx_status phx_set_params(phx_grid* g, const phx_params* p);
+
+/* Static real fields [ny][nx] of type T shared by the batch: potential V (Eq. (1)) and pump P
+ * (Eq. (17), P_+ = P_-).  NULL = identically zero.  The data are copied into the workspace. */
+phx_status phx_set_potential_pump(phx_grid* g, const void* V, const void* P, phx_mem where);
+
+/* Complex drive amplitude E(r) [ny][nx] (Eq. (16), E_+ = E_-); NULL = no drive. */
+phx_status phx_set_drive(phx_grid* g, const void* E, phx_mem where);
+
+/* Copies a state field [batch][ny][nx] into / out of the workspace.  phx_read_field synchronises
+ * the stream before returning.  UNSUPPORTED if the model does not have the field. */
+phx_status phx_set_field(phx_grid* g, phx_field f, const void* src, phx_mem where);
+phx_status phx_read_field(phx_grid* g, phx_field f, void* dst, phx_mem where);
+
+/* Advances every realisation by n_steps (>= 0) RK4 steps.  Asynchronous on the stream. */
+phx_status phx_step_rk4(phx_grid* g, int64_t n_steps);
+
+/* Step counter = number of completed steps.  phx_set_step synchronises. */
+phx_status phx_get_step(const phx_grid* g, uint64_t* step);
+phx_status phx_set_step(phx_grid* g, uint64_t step);
+
+/* <|psi|^2>(x,y) = (1/batch) sum_r |psi_r|^2 as real T [ny][nx].  Synchronises. */
+phx_status phx_ensemble_mean_density(phx_grid* g, phx_field f, void* dst, phx_mem where);
+
+/* The canonical coefficients actually used (as double); n must be PHX_NCOEF. */
+phx_status phx_get_coeffs(const phx_grid* g, double* out, int32_t n);
+
+/* Test aid: the four Philox4x32-10 words every (realisation, cell) draws at step `step`,
+ * dst[batch][ny][nx][4], produced by the same device function the stepping kernels call. */
+phx_status phx_debug_noise_u32(phx_grid* g, uint64_t step, uint32_t* dst, phx_mem where);
+
+/* Selects a kernel variant (phx_variant).  UNSUPPORTED if it cannot run this grid/model. */
+phx_status phx_select_variant(phx_grid* g, int32_t variant);
+
+/* Bench/test aids: the variant the next phx_step_rk4 will use; kernels launched so far by this handle;
+ * launch geometry knobs (key/value, UNSUPPORTED for unknown keys). */
+phx_status phx_get_variant(const phx_grid* g, int32_t* variant);
+phx_status phx_get_launch_count(const phx_grid* g, uint64_t* launches);
+phx_status phx_set_tuning(phx_grid* g, const char* key, int32_t value);
+
+/* Waits for the stream; returns the sticky CUDA status. */
+phx_status phx_sync(phx_grid* g);
+
+/* Human-readable description of the last error of this handle (never NULL). */
+const char* phx_last_error(const phx_grid* g);
+
+void phx_destroy_grid(phx_grid* g);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,540 @@
+// phx_api.cu -- the C ABI of libphx (include/phx.h): handle, validation, workspace carving, copies,
+// canonical coefficients, launch plan (CUDA graphs of the per-step kernel sequence).
+// There is no CPU path: every step of the method runs in the kernels of this library.
+#include "../../include/phx.h"
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+
+#include "phx_launch.h"
+#include "phx_stage.cuh"
+
+using namespace phx;
+
+namespace {
+
+constexpr size_t ALIGN = 256;
+inline size_t align_up(size_t v) { return (v + ALIGN - 1) / ALIGN * ALIGN; }
+
+struct Layout {
+    size_t psi[2], ya[2], yb[2], acc[2], n[2], na[2], nb[2], nacc[2], V, P, E, step, total;
+    size_t scratch_bytes;   // ya[0]..acc[0] are contiguous: usable as scratch between steps
+};
+
+bool desc_ok(const phx_grid_desc* d) {
+    if (!d) return false;
+    if (d->nx < 3 || d->ny < 3 || d->batch < 1 || d->batch > 65535) return false;
+    if (!(d->dx > 0) || !(d->dy > 0)) return false;
+    if (d->prec != PHX_C32 && d->prec != PHX_C64) return false;
+    if (d->model < PHX_SCALAR || d->model > PHX_SPINOR_RESERVOIR) return false;
+    if ((d->bc_x != 0 && d->bc_x != 1) || (d->bc_y != 0 && d->bc_y != 1)) return false;
+    if (d->noise != 0 && d->noise != 1) return false;
+    if ((size_t)d->nx * (size_t)d->ny > 0xffffffffull) return false;   // the noise counter holds the cell index in 32 bits
+    return true;
+}
+
+Layout make_layout(const phx_grid_desc* d) {
+    Layout L;
+    std::memset(&L, 0, sizeof(L));
+    const size_t rb = d->prec == PHX_C64 ? 8 : 4, cb = 2 * rb;
+    const size_t plane = (size_t)d->nx * d->ny, cells = plane * d->batch;
+    const int nc = model_spinor(d->model) ? 2 : 1;
+    const bool res = model_reservoir(d->model);
+    size_t off = 0;
+    auto take = [&](size_t bytes) { const size_t o = off; off += align_up(bytes); return o; };
+    for (int s = 0; s < nc; ++s) {
+        L.psi[s] = take(cells * cb);
+        L.ya[s] = take(cells * cb);
+        L.yb[s] = take(cells * cb);
+        L.acc[s] = take(cells * cb);
+    }
+    L.scratch_bytes = L.acc[0] + align_up(cells * cb) - L.ya[0];
+    if (res)
+        for (int s = 0; s < nc; ++s) {
+            L.n[s] = take(cells * rb);
+            L.na[s] = take(cells * rb);
+            L.nb[s] = take(cells * rb);
+            L.nacc[s] = take(cells * rb);
+        }
+    L.V = take(plane * rb);
+    L.P = take(plane * rb);
+    L.E = take(plane * cb);
+    L.step = take(ALIGN);
+    L.total = off;
+    return L;
+}
+
+}  // namespace
+
+struct phx_grid {
+    phx_grid_desc d;
+    Layout L;
+    char* ws;
+    cudaStream_t stream;
+    cudaStream_t cap_stream;
+    bool has_params;
+    phx_params prm;
+    double coef[PHX_NCOEF];
+    bool hasV, hasP, hasE;
+    uint64_t step_host;
+    uint64_t launches;
+    int variant;            // resolved variant used by the next step
+    int variant_req;        // requested (may be AUTO)
+    int rows, vec, graph_steps;
+    cudaGraphExec_t g1, gN;  // one step / graph_steps steps
+    bool graphs_valid;
+    cudaError_t sticky;
+    std::string err;
+};
+
+namespace {
+
+phx_status fail(phx_grid* g, phx_status st, const char* msg) {
+    if (g) g->err = msg;
+    return st;
+}
+
+phx_status cuda_fail(phx_grid* g, cudaError_t e, const char* where) {
+    if (g) {
+        g->sticky = e;
+        g->err = std::string(where) + ": " + cudaGetErrorString(e);
+    }
+    return PHX_ERR_CUDA;
+}
+
+#define PHX_CUDA(g, call)                                        \
+    do {                                                         \
+        cudaError_t e__ = (call);                                \
+        if (e__ != cudaSuccess) return cuda_fail(g, e__, #call); \
+    } while (0)
+
+size_t real_bytes(const phx_grid* g) { return g->d.prec == PHX_C64 ? 8 : 4; }
+size_t plane_cells(const phx_grid* g) { return (size_t)g->d.nx * g->d.ny; }
+
+bool field_present(const phx_grid* g, int f) {
+    const bool sp = model_spinor(g->d.model), rs = model_reservoir(g->d.model);
+    switch (f) {
+        case PHX_PSI: return true;
+        case PHX_PSI_MINUS: return sp;
+        case PHX_N: return rs;
+        case PHX_N_MINUS: return rs && sp;
+    }
+    return false;
+}
+
+void* field_ptr(phx_grid* g, int f, size_t* bytes) {
+    const size_t cells = plane_cells(g) * g->d.batch, rb = real_bytes(g);
+    switch (f) {
+        case PHX_PSI: *bytes = cells * 2 * rb; return g->ws + g->L.psi[0];
+        case PHX_PSI_MINUS: *bytes = cells * 2 * rb; return g->ws + g->L.psi[1];
+        case PHX_N: *bytes = cells * rb; return g->ws + g->L.n[0];
+        case PHX_N_MINUS: *bytes = cells * rb; return g->ws + g->L.n[1];
+    }
+    *bytes = 0;
+    return nullptr;
+}
+
+void drop_graphs(phx_grid* g) {
+    if (g->g1) cudaGraphExecDestroy(g->g1);
+    if (g->gN) cudaGraphExecDestroy(g->gN);
+    g->g1 = g->gN = nullptr;
+    g->graphs_valid = false;
+}
+
+template <typename T>
+void fill_args(const phx_grid* g, StageArgs<T>& a) {
+    using C = typename Cx<T>::type;
+    std::memset(&a, 0, sizeof(a));
+    a.geo.nx = g->d.nx; a.geo.ny = g->d.ny; a.geo.batch = g->d.batch;
+    a.geo.bc_x = g->d.bc_x; a.geo.bc_y = g->d.bc_y;
+    a.geo.rows = g->rows;
+    a.geo.plane = plane_cells(g);
+    const double* c = g->coef;
+    Coef<T>& k = a.k;
+    k.cx = (T)c[0]; k.cy = (T)c[1]; k.ih = (T)c[2]; k.g = (T)c[3]; k.gx = (T)c[4]; k.gr = (T)c[5]; k.Rr = (T)c[6];
+    k.hgc = (T)c[7]; k.gamr = (T)c[8]; k.bxx = (T)c[9]; k.byy = (T)c[10]; k.bxy = (T)c[11]; k.dt = (T)c[12];
+    k.hdt = (T)(0.5 * c[12]);           // exact
+    k.dt6 = (T)c[13]; k.dt3 = (T)c[14]; k.sig2 = (T)c[15]; k.doff = (T)c[16];
+    k.r13 = (T)(c[13] / (0.5 * c[12]));
+    k.omega = c[17];
+    k.dt_d = c[12];
+    const int nc = model_spinor(g->d.model) ? 2 : 1;
+    const bool res = model_reservoir(g->d.model);
+    for (int s = 0; s < nc; ++s) {
+        a.f.psi[s] = (C*)(g->ws + g->L.psi[s]);
+        a.f.ya[s] = (C*)(g->ws + g->L.ya[s]);
+        a.f.yb[s] = (C*)(g->ws + g->L.yb[s]);
+        a.f.acc[s] = (C*)(g->ws + g->L.acc[s]);
+        if (res) {
+            a.f.n[s] = (T*)(g->ws + g->L.n[s]);
+            a.f.na[s] = (T*)(g->ws + g->L.na[s]);
+            a.f.nb[s] = (T*)(g->ws + g->L.nb[s]);
+            a.f.nacc[s] = (T*)(g->ws + g->L.nacc[s]);
+        }
+    }
+    a.f.V = g->hasV ? (const T*)(g->ws + g->L.V) : nullptr;
+    a.f.P = g->hasP ? (const T*)(g->ws + g->L.P) : nullptr;
+    a.f.E = g->hasE ? (const C*)(g->ws + g->L.E) : nullptr;
+    a.f.step = (uint64_t*)(g->ws + g->L.step);
+    a.seed = g->prm.seed;
+}
+
+// One RK4 step of variant STAGE: four fused stage kernels.
+template <typename T>
+cudaError_t enqueue_step_stage(phx_grid* g, cudaStream_t st) {
+    StageArgs<T> a;
+    fill_args<T>(g, a);
+    const int vec = g->vec;
+    const int tx = (g->d.nx + vec - 1) / vec;                   // threads needed along x
+    int bx = ((tx + 31) / 32) * 32;
+    if (bx > 128) bx = 128;
+    const int by = 128 / bx;
+    const dim3 block(bx, by, 1);
+    const dim3 grid((tx + bx - 1) / bx, (g->d.ny + g->rows * by - 1) / (g->rows * by), g->d.batch);
+    if (grid.y > 65535u) return cudaErrorInvalidConfiguration;
+    for (int stage = 1; stage <= 4; ++stage) {
+        cudaError_t e;
+        const bool noise = g->d.noise != 0;
+        if constexpr (sizeof(T) == 4) {
+            switch (g->d.model) {
+                case 0: e = launch_stage_32_0(a, stage, noise, vec, grid, block, st); break;
+                case 1: e = launch_stage_32_1(a, stage, noise, vec, grid, block, st); break;
+                case 2: e = launch_stage_32_2(a, stage, noise, vec, grid, block, st); break;
+                default: e = launch_stage_32_3(a, stage, noise, vec, grid, block, st); break;
+            }
+        } else {
+            switch (g->d.model) {
+                case 0: e = launch_stage_64_0(a, stage, noise, vec, grid, block, st); break;
+                case 1: e = launch_stage_64_1(a, stage, noise, vec, grid, block, st); break;
+                case 2: e = launch_stage_64_2(a, stage, noise, vec, grid, block, st); break;
+                default: e = launch_stage_64_3(a, stage, noise, vec, grid, block, st); break;
+            }
+        }
+        if (e != cudaSuccess) return e;
+    }
+    return cudaSuccess;
+}
+
+int kernels_per_step(const phx_grid* g) { return g->variant == PHX_VARIANT_STAGE ? 4 : 4; }
+
+cudaError_t enqueue_step(phx_grid* g, cudaStream_t st) {
+    return g->d.prec == PHX_C64 ? enqueue_step_stage<double>(g, st) : enqueue_step_stage<float>(g, st);
+}
+
+cudaError_t capture(phx_grid* g, int steps, cudaGraphExec_t* out) {
+    cudaGraph_t graph = nullptr;
+    cudaError_t e = cudaStreamBeginCapture(g->cap_stream, cudaStreamCaptureModeThreadLocal);
+    if (e != cudaSuccess) return e;
+    cudaError_t le = cudaSuccess;
+    for (int s = 0; s < steps && le == cudaSuccess; ++s) le = enqueue_step(g, g->cap_stream);
+    e = cudaStreamEndCapture(g->cap_stream, &graph);
+    if (le != cudaSuccess) { if (graph) cudaGraphDestroy(graph); return le; }
+    if (e != cudaSuccess) return e;
+    e = cudaGraphInstantiate(out, graph, 0);
+    cudaGraphDestroy(graph);
+    return e;
+}
+
+void resolve_variant(phx_grid* g) {
+    g->variant = PHX_VARIANT_STAGE;   // the only variant that runs every model / size
+    if (g->variant_req == PHX_VARIANT_STAGE) g->variant = PHX_VARIANT_STAGE;
+}
+
+phx_status copy_in(phx_grid* g, void* dst, const void* src, size_t bytes, phx_mem where) {
+    if (where == PHX_HOST) {
+        PHX_CUDA(g, cudaMemcpyAsync(dst, src, bytes, cudaMemcpyHostToDevice, g->stream));
+        PHX_CUDA(g, cudaStreamSynchronize(g->stream));   // the caller may reuse a pageable source at once
+    } else {
+        PHX_CUDA(g, cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToDevice, g->stream));
+    }
+    return PHX_OK;
+}
+
+phx_status copy_out(phx_grid* g, void* dst, const void* src, size_t bytes, phx_mem where) {
+    PHX_CUDA(g, cudaMemcpyAsync(dst, src, bytes, where == PHX_HOST ? cudaMemcpyDeviceToHost : cudaMemcpyDeviceToDevice,
+                                g->stream));
+    PHX_CUDA(g, cudaStreamSynchronize(g->stream));
+    return PHX_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+size_t phx_workspace_bytes(const phx_grid_desc* desc) {
+    if (!desc_ok(desc)) return 0;
+    return make_layout(desc).total;
+}
+
+phx_status phx_create_grid(phx_grid** out, const phx_grid_desc* desc) {
+    if (!out) return PHX_ERR_INVALID_ARG;
+    *out = nullptr;
+    if (!desc_ok(desc)) return PHX_ERR_INVALID_ARG;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) return PHX_ERR_CUDA;   // no CPU fallback
+    int dev = 0;
+    cudaDeviceProp prop;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) return PHX_ERR_CUDA;
+    if (prop.major != 10) return PHX_ERR_CUDA;   // the kernels are built for sm_100a only
+    const Layout L = make_layout(desc);
+    if (!desc->workspace || ((uintptr_t)desc->workspace % ALIGN) != 0 || desc->workspace_bytes < L.total)
+        return PHX_ERR_WORKSPACE;
+    cudaPointerAttributes attr;
+    if (cudaPointerGetAttributes(&attr, desc->workspace) != cudaSuccess || attr.type != cudaMemoryTypeDevice) {
+        cudaGetLastError();
+        return PHX_ERR_WORKSPACE;
+    }
+    phx_grid* g = new (std::nothrow) phx_grid();
+    if (!g) return PHX_ERR_INVALID_ARG;
+    g->d = *desc;
+    g->L = L;
+    g->ws = (char*)desc->workspace;
+    g->stream = (cudaStream_t)desc->stream;
+    g->cap_stream = nullptr;
+    g->has_params = false;
+    std::memset(&g->prm, 0, sizeof(g->prm));
+    std::memset(g->coef, 0, sizeof(g->coef));
+    g->hasV = g->hasP = g->hasE = false;
+    g->step_host = 0;
+    g->launches = 0;
+    g->variant_req = PHX_VARIANT_AUTO;
+    g->rows = 16;
+    g->vec = (desc->prec == PHX_C32 && desc->nx % 2 == 0) ? 2 : 1;
+    g->graph_steps = 8;
+    g->g1 = g->gN = nullptr;
+    g->graphs_valid = false;
+    g->sticky = cudaSuccess;
+    resolve_variant(g);
+    if (cudaStreamCreateWithFlags(&g->cap_stream, cudaStreamNonBlocking) != cudaSuccess) { delete g; return PHX_ERR_CUDA; }
+    // zero the state, the static fields and the step counter
+    if (cudaMemsetAsync(g->ws, 0, L.total, g->stream) != cudaSuccess) { cudaStreamDestroy(g->cap_stream); delete g; return PHX_ERR_CUDA; }
+    *out = g;
+    return PHX_OK;
+}
+
+phx_status phx_set_params(phx_grid* g, const phx_params* p) {
+    if (!g || !p) return PHX_ERR_INVALID_ARG;
+    if (g->sticky != cudaSuccess) return PHX_ERR_CUDA;
+    if (!(p->dt > 0) || p->hbar == 0 || p->m == 0 || !std::isfinite(p->hbar) || !std::isfinite(p->m) || !std::isfinite(p->dt))
+        return fail(g, PHX_ERR_INVALID_ARG, "phx_set_params: dt must be > 0 and hbar, m non-zero");
+    const double dx = g->d.dx, dy = g->d.dy;
+    double c[PHX_NCOEF];
+    // canonical coefficient set (step 0): double expressions, each rounded once to T
+    c[0] = p->hbar / (2.0 * p->m * dx * dx);
+    c[1] = p->hbar / (2.0 * p->m * dy * dy);
+    c[2] = 1.0 / p->hbar;
+    c[3] = p->g;
+    c[4] = p->g_x;
+    c[5] = p->g_r;
+    c[6] = p->R;
+    c[7] = p->gamma_c / 2.0;
+    c[8] = p->gamma_r;
+    c[9] = p->beta / (p->hbar * dx * dx);
+    c[10] = p->beta / (p->hbar * dy * dy);
+    c[11] = p->beta / (2.0 * p->hbar * dx * dy);
+    c[12] = p->dt;
+    c[13] = p->dt / 6.0;
+    c[14] = p->dt / 3.0;
+    c[15] = p->noise_scale * p->dt / (4.0 * dx * dy);
+    c[16] = p->density_offset;
+    c[17] = p->omega;
+    for (int i = 0; i < PHX_NCOEF; ++i) {
+        if (!std::isfinite(c[i])) return fail(g, PHX_ERR_INVALID_ARG, "phx_set_params: non-finite coefficient");
+        g->coef[i] = g->d.prec == PHX_C32 ? (double)(float)c[i] : c[i];
+    }
+    g->prm = *p;
+    g->has_params = true;
+    drop_graphs(g);
+    const double wmax = std::fabs(p->hbar / (2.0 * p->m)) * (4.0 / (dx * dx) + 4.0 / (dy * dy)) * p->dt;
+    if (wmax > 2.78) {
+        g->err = "phx_set_params: (hbar/2m)(4/dx^2+4/dy^2) dt exceeds the RK4 stability limit 2.78";
+        return PHX_WARN_UNSTABLE;
+    }
+    return PHX_OK;
+}
+
+phx_status phx_set_potential_pump(phx_grid* g, const void* V, const void* P, phx_mem where) {
+    if (!g || (where != PHX_HOST && where != PHX_DEVICE)) return PHX_ERR_INVALID_ARG;
+    if (g->sticky != cudaSuccess) return PHX_ERR_CUDA;
+    const size_t bytes = plane_cells(g) * real_bytes(g);
+    if (V) { phx_status s = copy_in(g, g->ws + g->L.V, V, bytes, where); if (s) return s; }
+    if (P) { phx_status s = copy_in(g, g->ws + g->L.P, P, bytes, where); if (s) return s; }
+    if (g->hasV != (V != nullptr) || g->hasP != (P != nullptr)) drop_graphs(g);
+    g->hasV = V != nullptr;
+    g->hasP = P != nullptr;
+    return PHX_OK;
+}
+
+phx_status phx_set_drive(phx_grid* g, const void* E, phx_mem where) {
+    if (!g || (where != PHX_HOST && where != PHX_DEVICE)) return PHX_ERR_INVALID_ARG;
+    if (g->sticky != cudaSuccess) return PHX_ERR_CUDA;
+    if (E) { phx_status s = copy_in(g, g->ws + g->L.E, E, plane_cells(g) * 2 * real_bytes(g), where); if (s) return s; }
+    if (g->hasE != (E != nullptr)) drop_graphs(g);
+    g->hasE = E != nullptr;
+    return PHX_OK;
+}
+
+phx_status phx_set_field(phx_grid* g, phx_field f, const void* src, phx_mem where) {
+    if (!g || !src || (where != PHX_HOST && where != PHX_DEVICE) || f < PHX_PSI || f > PHX_N_MINUS) return PHX_ERR_INVALID_ARG;
+    if (g->sticky != cudaSuccess) return PHX_ERR_CUDA;
+    if (!field_present(g, f)) return fail(g, PHX_ERR_UNSUPPORTED, "phx_set_field: field not present in this model");
+    size_t bytes;
+    void* dst = field_ptr(g, f, &bytes);
+    return copy_in(g, dst, src, bytes, where);
+}
+
+phx_status phx_read_field(phx_grid* g, phx_field f, void* dst, phx_mem where) {
+    if (!g || !dst || (where != PHX_HOST && where != PHX_DEVICE) || f < PHX_PSI || f > PHX_N_MINUS) return PHX_ERR_INVALID_ARG;
+    if (g->sticky != cudaSuccess) return PHX_ERR_CUDA;
+    if (!field_present(g, f)) return fail(g, PHX_ERR_UNSUPPORTED, "phx_read_field: field not present in this model");
+    size_t bytes;
+    void* src = field_ptr(g, f, &bytes);
+    return copy_out(g, dst, src, bytes, where);
+}
+
+phx_status phx_step_rk4(phx_grid* g, int64_t n_steps) {
+    if (!g || n_steps < 0) return PHX_ERR_INVALID_ARG;
+    if (g->sticky != cudaSuccess) return PHX_ERR_CUDA;
+    if (!g->has_params) return fail(g, PHX_ERR_BAD_STATE, "phx_step_rk4: call phx_set_params first");
+    if (n_steps == 0) return PHX_OK;
+    if (!g->graphs_valid) {
+        drop_graphs(g);
+        PHX_CUDA(g, capture(g, 1, &g->g1));
+        PHX_CUDA(g, capture(g, g->graph_steps, &g->gN));
+        g->graphs_valid = true;
+    }
+    int64_t left = n_steps;
+    while (left >= g->graph_steps) {
+        PHX_CUDA(g, cudaGraphLaunch(g->gN, g->stream));
+        left -= g->graph_steps;
+    }
+    while (left > 0) {
+        PHX_CUDA(g, cudaGraphLaunch(g->g1, g->stream));
+        --left;
+    }
+    g->step_host += (uint64_t)n_steps;
+    g->launches += (uint64_t)n_steps * kernels_per_step(g);
+    return PHX_OK;
+}
+
+phx_status phx_get_step(const phx_grid* g, uint64_t* step) {
+    if (!g || !step) return PHX_ERR_INVALID_ARG;
+    *step = g->step_host;
+    return PHX_OK;
+}
+
+phx_status phx_set_step(phx_grid* g, uint64_t step) {
+    if (!g) return PHX_ERR_INVALID_ARG;
+    if (g->sticky != cudaSuccess) return PHX_ERR_CUDA;
+    const uint64_t slots[2] = {step, step};
+    PHX_CUDA(g, cudaMemcpyAsync(g->ws + g->L.step, slots, sizeof(slots), cudaMemcpyHostToDevice, g->stream));
+    PHX_CUDA(g, cudaStreamSynchronize(g->stream));
+    g->step_host = step;
+    return PHX_OK;
+}
+
+phx_status phx_ensemble_mean_density(phx_grid* g, phx_field f, void* dst, phx_mem where) {
+    if (!g || !dst || (where != PHX_HOST && where != PHX_DEVICE)) return PHX_ERR_INVALID_ARG;
+    if (g->sticky != cudaSuccess) return PHX_ERR_CUDA;
+    if (f != PHX_PSI && f != PHX_PSI_MINUS) return PHX_ERR_INVALID_ARG;
+    if (!field_present(g, f)) return fail(g, PHX_ERR_UNSUPPORTED, "phx_ensemble_mean_density: field not present");
+    size_t bytes;
+    void* psi = field_ptr(g, f, &bytes);
+    void* scratch = g->ws + g->L.ya[0];   // stage buffers are dead between steps
+    PHX_CUDA(g, launch_ensemble_mean(psi, scratch, g->d.prec == PHX_C64, plane_cells(g), g->d.batch, g->stream));
+    g->launches += 1;
+    return copy_out(g, dst, scratch, plane_cells(g) * real_bytes(g), where);
+}
+
+phx_status phx_get_coeffs(const phx_grid* g, double* out, int32_t n) {
+    if (!g || !out || n != PHX_NCOEF) return PHX_ERR_INVALID_ARG;
+    if (!g->has_params) return PHX_ERR_BAD_STATE;
+    std::memcpy(out, g->coef, sizeof(double) * PHX_NCOEF);
+    return PHX_OK;
+}
+
+phx_status phx_debug_noise_u32(phx_grid* g, uint64_t step, uint32_t* dst, phx_mem where) {
+    if (!g || !dst || (where != PHX_HOST && where != PHX_DEVICE)) return PHX_ERR_INVALID_ARG;
+    if (g->sticky != cudaSuccess) return PHX_ERR_CUDA;
+    if (!g->has_params) return fail(g, PHX_ERR_BAD_STATE, "phx_debug_noise_u32: call phx_set_params first (seed)");
+    const size_t plane = plane_cells(g);
+    if (where == PHX_DEVICE) {
+        PHX_CUDA(g, launch_noise_words(dst, g->prm.seed, step, plane, 0, g->d.batch, g->stream));
+        PHX_CUDA(g, cudaStreamSynchronize(g->stream));
+        return PHX_OK;
+    }
+    // stage through the (dead between steps) stage buffers, one chunk of realisations at a time
+    const size_t per_real = plane * 16;
+    const size_t chunk = g->L.scratch_bytes / per_real;
+    if (chunk < 1) return fail(g, PHX_ERR_UNSUPPORTED, "phx_debug_noise_u32: scratch too small");
+    uint32_t* scratch = (uint32_t*)(g->ws + g->L.ya[0]);
+    for (size_t r0 = 0; r0 < (size_t)g->d.batch; r0 += chunk) {
+        const size_t nr = (size_t)g->d.batch - r0 < chunk ? (size_t)g->d.batch - r0 : chunk;
+        PHX_CUDA(g, launch_noise_words(scratch, g->prm.seed, step, plane, (int)r0, (int)nr, g->stream));
+        phx_status s = copy_out(g, dst + r0 * plane * 4, scratch, nr * per_real, PHX_HOST);
+        if (s) return s;
+    }
+    return PHX_OK;
+}
+
+phx_status phx_select_variant(phx_grid* g, int32_t variant) {
+    if (!g) return PHX_ERR_INVALID_ARG;
+    if (variant != PHX_VARIANT_AUTO && variant != PHX_VARIANT_STAGE)
+        return fail(g, PHX_ERR_UNSUPPORTED, "phx_select_variant: variant not available for this grid/model");
+    g->variant_req = variant;
+    resolve_variant(g);
+    drop_graphs(g);
+    return PHX_OK;
+}
+
+phx_status phx_get_variant(const phx_grid* g, int32_t* variant) {
+    if (!g || !variant) return PHX_ERR_INVALID_ARG;
+    *variant = g->variant;
+    return PHX_OK;
+}
+
+phx_status phx_get_launch_count(const phx_grid* g, uint64_t* launches) {
+    if (!g || !launches) return PHX_ERR_INVALID_ARG;
+    *launches = g->launches;
+    return PHX_OK;
+}
+
+phx_status phx_set_tuning(phx_grid* g, const char* key, int32_t value) {
+    if (!g || !key) return PHX_ERR_INVALID_ARG;
+    if (!std::strcmp(key, "rows")) {
+        if (value < 1 || value > 4096) return PHX_ERR_INVALID_ARG;
+        g->rows = value;
+    } else if (!std::strcmp(key, "vec")) {
+        if (value != 1 && value != 2) return PHX_ERR_INVALID_ARG;
+        if (value == 2 && g->d.nx % 2 != 0) return fail(g, PHX_ERR_UNSUPPORTED, "vec=2 needs even nx");
+        g->vec = value;
+    } else if (!std::strcmp(key, "graph_steps")) {
+        if (value < 1 || value > 256) return PHX_ERR_INVALID_ARG;
+        g->graph_steps = value;
+    } else {
+        return fail(g, PHX_ERR_UNSUPPORTED, "phx_set_tuning: unknown key");
+    }
+    drop_graphs(g);
+    return PHX_OK;
+}
+
+phx_status phx_sync(phx_grid* g) {
+    if (!g) return PHX_ERR_INVALID_ARG;
+    if (g->sticky != cudaSuccess) return PHX_ERR_CUDA;
+    PHX_CUDA(g, cudaStreamSynchronize(g->stream));
+    return PHX_OK;
+}
+
+const char* phx_last_error(const phx_grid* g) { return g ? g->err.c_str() : "null handle"; }
+
+void phx_destroy_grid(phx_grid* g) {
+    if (!g) return;
+    drop_graphs(g);
+    if (g->cap_stream) cudaStreamDestroy(g->cap_stream);
+    delete g;
+}
+
+}  // extern "C"

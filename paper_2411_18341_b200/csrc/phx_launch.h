@@ -1,0 +1,23 @@
+// phx_launch.h -- host-side entry points of the kernel translation units (internal to libphx).
+#pragma once
+
+#include "phx_common.cuh"
+
+namespace phx {
+
+template <typename T> struct StageArgs;
+
+#define PHX_DECL_STAGE(P, T)                                                                                              \
+    cudaError_t launch_stage_##P##_0(const StageArgs<T>&, int stage, bool noise, int vec, dim3 grid, dim3 block, cudaStream_t); \
+    cudaError_t launch_stage_##P##_1(const StageArgs<T>&, int stage, bool noise, int vec, dim3 grid, dim3 block, cudaStream_t); \
+    cudaError_t launch_stage_##P##_2(const StageArgs<T>&, int stage, bool noise, int vec, dim3 grid, dim3 block, cudaStream_t); \
+    cudaError_t launch_stage_##P##_3(const StageArgs<T>&, int stage, bool noise, int vec, dim3 grid, dim3 block, cudaStream_t);
+PHX_DECL_STAGE(32, float)
+PHX_DECL_STAGE(64, double)
+#undef PHX_DECL_STAGE
+
+// phx_aux.cu: small helper kernels
+cudaError_t launch_ensemble_mean(const void* psi, void* out, int prec64, size_t plane, int batch, cudaStream_t);
+cudaError_t launch_noise_words(uint32_t* out, uint32_t seed, uint64_t step, size_t plane, int r0, int batch, cudaStream_t);
+
+}  // namespace phx

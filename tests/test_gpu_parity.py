@@ -5,7 +5,7 @@ import numpy as np
 import pytest
 
 from paper_2411_18341_b200 import workloads as wl
-from tests.helpers import TOL, compare, make_gpu, make_oracle, rel_l2
+from helpers import TOL, compare, make_gpu, make_oracle, rel_l2
 
 pytestmark = pytest.mark.gpu
 

@@ -1,0 +1,330 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the RK4 hot path on B200 (BASELINE.json metric: grid-cell RK4 steps per second).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload NAME] [--variant V] [--impl reference]
+
+A "step" is one RK4 step (all four stages, plus noise where the workload has it) over the whole grid /
+ensemble.  `value` times K steps with the state resident in HBM (CUDA events on the launching stream,
+barrier + synchronize on both sides, max over ranks).  `e2e` times the same metric through the C ABI with
+HOST buffers: every step uploads psi from pinned host memory, runs one RK4 step and downloads psi.
+The path does not shard (replicas only): with --gpus N each rank steps an independent
+replica of the workload and `value` is the sum.  Prints ONE JSON line on rank 0.
+"""
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+METRIC = "grid-cell RK4 steps/sec"
+UNIT = "Gcell*step/s"
+
+# Compulsory (infinite-cache) bytes per cell-step, fp32 (fp64: x2); DESIGN.md section 6.
+COMPULSORY_BYTES = {"scalar": 20, "reservoir": 28, "spinor": 32, "spinor_reservoir": 52}
+
+
+def build_workload(name):
+    from paper_2411_18341_b200 import workloads as wl
+    table = {
+        "cfg1": lambda: wl.cfg1(),
+        "cfg2_1024_c32": lambda: wl.cfg2(1024, "c32"), "cfg2_1024_c64": lambda: wl.cfg2(1024, "c64"),
+        "cfg2_4096_c32": lambda: wl.cfg2(4096, "c32"), "cfg2_4096_c64": lambda: wl.cfg2(4096, "c64"),
+        "cfg3_4096_c32": lambda: wl.cfg3(4096, "c32"),
+        "cfg4_16384_c32": lambda: wl.cfg4(16384, "c32"), "cfg4_8192_c32": lambda: wl.cfg4(8192, "c32"),
+        "cfg5_512x256_c32": lambda: wl.cfg5(256, 512, "c32"),
+    }
+    if name not in table:
+        raise SystemExit(f"unknown workload {name}; choose from {sorted(table)}")
+    return table[name]()
+
+
+def algo_bytes_per_cell_step(w, variant):
+    """Algorithmic HBM bytes per cell-step of variant STAGE, counted array by array.
+
+    Per complex component: s1 R psi, W y2; s2 R y2, psi, W y3, acc; s3 R y3, psi, acc, W y4, acc;
+    s4 R y4, acc, W psi = 14 complex transfers.  Per reservoir: s1 R n, W n2; s2 R n2, n, W n3, nacc;
+    s3 R n3, n, nacc, W n4, nacc; s4 R n4, nacc, W n = 14 real transfers.  V, P: one real read per stage."""
+    rb = 8 if w.prec == "c64" else 4
+    ncomp = 2 if w.model.startswith("spinor") else 1
+    res = w.model.endswith("reservoir")
+    b = ncomp * 14 * 2 * rb
+    if res:
+        b += ncomp * 14 * rb
+        if w.P is not None:
+            b += 4 * rb
+        if w.noise:
+            b += ncomp * rb                                 # n_t re-read for sigma (Eq. 22)
+    if w.V is not None:
+        b += 4 * rb
+    return b
+
+
+class ClockSampler:
+    """Samples nvidia-smi clocks and throttle reasons while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100",
+                                          "-i", str(self.index)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.time(), line.strip()))
+
+    def stop(self, t0, t1):
+        if self.proc is None:
+            return None
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons, pw = [], [], set(), []
+        rows = [r for r in self.rows if t0 <= r[0] <= t1 + 0.2] or self.rows[-3:]
+        for _, line in rows:
+            p = [v.strip() for v in line.split(",")]
+            try:
+                sm.append(float(p[0])); mx.append(float(p[1])); pw.append(float(p[2]))
+            except Exception:
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), p[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        if not sm:
+            return None
+        return {"sm_mhz": statistics.median(sm), "sm_max_mhz": max(mx), "power_w_max": max(pw), "samples": len(sm),
+                "reasons": sorted(reasons)}
+
+
+def measured_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        try:
+            return float(json.load(open(path))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def oracle_from_workload(w, ny=None):
+    """The oracle as it stands on (a row-slab sample of) the workload."""
+    import oracle as orc
+    ny = w.ny if ny is None else ny
+    o = orc.Oracle(w.nx, ny, w.dx, w.dy, orc.make_params(**w.params), model=w.model, batch=1, prec32=(w.prec == "c32"),
+                   noise=w.noise, seed=w.seed, V=None if w.V is None else w.V[:ny].astype(np.float64),
+                   P=None if w.P is None else w.P[:ny].astype(np.float64))
+    for name, arr in w.fields.items():
+        o.set_field(name, arr[:1, :ny])
+    return o
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle, as it stands, on a bounded sample of the same workload."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    w = build_workload(args.workload)
+    # bounded sample: ~60 s of single-thread oracle work (~7 Mcell*step/s) over the whole run
+    target_cells = int(4.0e8 / max(1, args.steps + args.warmup))
+    ny = max(8, min(w.ny, target_cells // w.nx))
+    o = oracle_from_workload(w, ny)
+    for _ in range(args.warmup):
+        o.step_rk4(1)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        o.step_rk4(1)
+    dt = time.perf_counter() - t0
+    cells = w.nx * ny
+    val = cells * args.steps / dt / 1e9
+    sample = f"{w.nx}x{ny} row slab of realisation 0 (periodic), 1 RK4 step per bench step"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": args.workload, "sample": sample},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=2000)
+    ap.add_argument("--warmup", type=int, default=50)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="cfg2_4096_c32")
+    ap.add_argument("--variant", type=int, default=0)
+    ap.add_argument("--tune", default="", help="comma separated key=value passed to phx_set_tuning")
+    ap.add_argument("--e2e-steps", type=int, default=20)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    if args.warmup < 3:
+        args.warmup = 3
+
+    import torch
+    import torch.distributed as dist
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    from paper_2411_18341_b200 import binding as phx
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    w = build_workload(args.workload)
+    stream = torch.cuda.Stream()
+    g = phx.grid_from_workload(w, variant=args.variant, stream=stream, device=f"cuda:{local}")
+    for kv in filter(None, args.tune.split(",")):
+        k, v = kv.split("=")
+        g.set_tuning(k, int(v))
+    variant = g.get_variant()
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    # ---- device-resident throughput ---------------------------------------------------------------------
+    g.step_rk4(args.warmup)
+    barrier()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+        time.sleep(0.25)
+    launches0 = g.get_launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    t_wall0 = time.time()
+    e0.record(stream)
+    g.step_rk4(args.steps)
+    e1.record(stream)
+    barrier()
+    t_wall1 = time.time()
+    ms = e0.elapsed_time(e1)
+    launches = g.get_launch_count() - launches0
+    clocks = sampler.stop(t_wall0, t_wall1) if rank == 0 else None
+    if world > 1:
+        t = torch.tensor([ms], device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    cells = w.cells
+    value = world * cells * args.steps / (ms * 1e-3) / 1e9
+    finite = bool(np.all(np.isfinite(g.read_field("psi_p")[0, :4])))
+
+    # ---- end to end through the C ABI with host buffers ----------------------------------------------------
+    host_in = {k: torch.from_numpy(np.ascontiguousarray(v)).pin_memory() for k, v in w.fields.items()}
+    host_out = {k: torch.empty_like(v).pin_memory() for k, v in host_in.items()}
+    h2d = sum(v.numel() * v.element_size() for v in host_in.values())
+    d2h = h2d
+
+    def e2e_step():
+        for k, v in host_in.items():
+            g.set_field(k, v)
+        g.step_rk4(1)
+        for k, v in host_out.items():
+            g.read_field(k, v)
+    for _ in range(3):
+        e2e_step()
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(args.e2e_steps):
+        e2e_step()
+    barrier()
+    e2e_s = time.perf_counter() - t0
+    if world > 1:
+        t = torch.tensor([e2e_s], device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_s = float(t.item())
+    e2e_val = world * cells * args.e2e_steps / e2e_s / 1e9
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline of the dominant kernel ------------------------------------------------------------------------
+    peak, peak_src = measured_peaks()
+    bpc = algo_bytes_per_cell_step(w, variant)
+    kernels_per_step = launches / args.steps
+    bytes_per_launch = bpc * cells / kernels_per_step
+    launch_ms = ms / launches
+    achieved = bytes_per_launch / (launch_ms * 1e-3) / 1e9
+    comp = COMPULSORY_BYTES[w.model] * (2 if w.prec == "c64" else 1)
+    roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                "traffic": None, "peak_source": peak_src, "kernel": {1: "phx::stage_kernel (4 launches per step)"}.get(variant, str(variant)),
+                "algorithmic_bytes_per_cell_step": bpc, "bytes_per_launch": bytes_per_launch,
+                "avg_launch_ms": launch_ms, "compulsory_bytes_per_cell_step": comp,
+                "compulsory_frac": value / world * 1e9 * comp / 1e9 / peak}
+    traffic_file = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(traffic_file):
+        try:
+            tr = json.load(open(traffic_file)).get(f"{args.workload}:v{variant}")
+            if tr:
+                roofline["traffic"] = tr["dram_bytes_per_launch"]
+                roofline["traffic_source"] = tr["source"]
+        except Exception:
+            pass
+
+    # ---- the oracle timed on this box's host cores (bounded sample) -----------------------------------------------
+    cpu = None
+    if not args.no_cpu_baseline and world == 1:
+        ny = max(3, min(w.ny, (1 << 22) // w.nx))              # ~4M cells per step, ~0.4 s per step
+        o = oracle_from_workload(w, ny)
+        o.step_rk4(1)
+        t0 = time.perf_counter()
+        nst = 0
+        while time.perf_counter() - t0 < 12.0:
+            o.step_rk4(1)
+            nst += 1
+        dtc = time.perf_counter() - t0
+        cpu = {"value": w.nx * ny * nst / dtc / 1e9, "unit": UNIT, "cores": 1, "kind": "oracle",
+               "sample": f"{w.nx}x{ny} row slab of realisation 0, {nst} RK4 steps, fp64, single thread"}
+
+    out = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32" if w.prec == "c32" else "f64", "data": "synthetic",
+        "config": {"workload": args.workload, "model": None, "grid": [w.nx, w.ny], "batch": w.batch, "precision": w.prec,
+                   "variant": variant, "parallelism": "replicas only" if world > 1 else "single GPU",
+                   "l2": f"working set {g.workspace.numel() / 2**20:.0f} MiB > 126 MB L2, no flush needed"
+                   if g.workspace.numel() > 200e6 else "working set fits L2 (L2-resident regime, reported as such)",
+                   "finite": finite},
+        "clocks": clocks, "gpu_launches": int(launches),
+        "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                "rk4_steps_per_call": 1, "steps": args.e2e_steps},
+        "roofline": roofline, "cpu_baseline": cpu,
+    }
+    del out["config"]["model"]
+    print(json.dumps(out))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

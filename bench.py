@@ -56,6 +56,12 @@ def algo_bytes_per_cell_step(w, variant):
     rb = 8 if w.prec == "c64" else 4
     ncomp = 2 if w.model.startswith("spinor") else 1
     res = w.model.endswith("reservoir")
+    if variant == 3:
+        # variant STEP: every state array is read once and written once per step; V, P read once
+        b = ncomp * 2 * 2 * rb + (ncomp * 2 * rb if res else 0)
+        b += rb if w.V is not None else 0
+        b += rb if (res and w.P is not None) else 0
+        return b
     b = ncomp * 14 * 2 * rb
     if res:
         b += ncomp * 14 * rb
@@ -277,7 +283,7 @@ def main():
     achieved = bytes_per_launch / (launch_ms * 1e-3) / 1e9
     comp = COMPULSORY_BYTES[w.model] * (2 if w.prec == "c64" else 1)
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": None, "peak_source": peak_src, "kernel": {1: "phx::stage_kernel (4 launches per step)"}.get(variant, str(variant)),
+                "traffic": None, "peak_source": peak_src, "kernel": {1: "phx::stage_kernel (4 launches per step)", 3: "phx::step_kernel (1 launch per step)"}.get(variant, str(variant)),
                 "algorithmic_bytes_per_cell_step": bpc, "bytes_per_launch": bytes_per_launch,
                 "avg_launch_ms": launch_ms, "compulsory_bytes_per_cell_step": comp,
                 "compulsory_frac": value / world * 1e9 * comp / 1e9 / peak}

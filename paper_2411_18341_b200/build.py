@@ -26,7 +26,9 @@ def _units():
         for model in range(4):
             u.append((f"phx_stage_{prec}_{model}.o", "phx_stage_inst.cu",
                       [f"-DPHX_INST_PREC={prec}", f"-DPHX_INST_MODEL={model}"]))
-    for extra in ("phx_step.cu", "phx_resident.cu"):
+            u.append((f"phx_step_{prec}_{model}.o", "phx_step_inst.cu",
+                      [f"-DPHX_INST_PREC={prec}", f"-DPHX_INST_MODEL={model}"]))
+    for extra in ("phx_resident.cu",):
         if os.path.exists(os.path.join(CSRC, extra)):
             u.append((extra.replace(".cu", ".o"), extra, []))
     return u

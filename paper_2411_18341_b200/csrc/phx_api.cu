@@ -11,6 +11,7 @@
 
 #include "phx_launch.h"
 #include "phx_stage.cuh"
+#include "phx_step.cuh"
 
 using namespace phx;
 
@@ -21,7 +22,7 @@ inline size_t align_up(size_t v) { return (v + ALIGN - 1) / ALIGN * ALIGN; }
 
 struct Layout {
     size_t psi[2], ya[2], yb[2], acc[2], n[2], na[2], nb[2], nacc[2], V, P, E, step, total;
-    size_t scratch_bytes;   // ya[0]..acc[0] are contiguous: usable as scratch between steps
+    size_t scratch_bytes;   // yb[0], acc[0] are contiguous and dead between steps in every variant: scratch
 };
 
 bool desc_ok(const phx_grid_desc* d) {
@@ -51,7 +52,7 @@ Layout make_layout(const phx_grid_desc* d) {
         L.yb[s] = take(cells * cb);
         L.acc[s] = take(cells * cb);
     }
-    L.scratch_bytes = L.acc[0] + align_up(cells * cb) - L.ya[0];
+    L.scratch_bytes = L.acc[0] + align_up(cells * cb) - L.yb[0];
     if (res)
         for (int s = 0; s < nc; ++s) {
             L.n[s] = take(cells * rb);
@@ -83,9 +84,12 @@ struct phx_grid {
     uint64_t launches;
     int variant;            // resolved variant used by the next step
     int variant_req;        // requested (may be AUTO)
-    int rows, vec, graph_steps;
-    cudaGraphExec_t g1, gN;  // one step / graph_steps steps
+    int rows, vec, graph_steps, gsteps;
+    int parity;             // variant STEP ping-pongs the state: 0 = state in psi/n, 1 = state in ya/na
+    int step_ly, step_vec;  // variant STEP geometry (0 = automatic)
+    cudaGraphExec_t g1[2], gN;  // one step from parity 0 / 1; graph_steps steps from parity 0
     bool graphs_valid;
+    int n_sm;
     cudaError_t sticky;
     std::string err;
 };
@@ -125,35 +129,37 @@ bool field_present(const phx_grid* g, int f) {
     return false;
 }
 
+// Where the state field lives now (variant STEP alternates between the state buffer and the first stage buffer).
 void* field_ptr(phx_grid* g, int f, size_t* bytes) {
     const size_t cells = plane_cells(g) * g->d.batch, rb = real_bytes(g);
+    const bool alt = g->parity != 0;
     switch (f) {
-        case PHX_PSI: *bytes = cells * 2 * rb; return g->ws + g->L.psi[0];
-        case PHX_PSI_MINUS: *bytes = cells * 2 * rb; return g->ws + g->L.psi[1];
-        case PHX_N: *bytes = cells * rb; return g->ws + g->L.n[0];
-        case PHX_N_MINUS: *bytes = cells * rb; return g->ws + g->L.n[1];
+        case PHX_PSI: *bytes = cells * 2 * rb; return g->ws + (alt ? g->L.ya[0] : g->L.psi[0]);
+        case PHX_PSI_MINUS: *bytes = cells * 2 * rb; return g->ws + (alt ? g->L.ya[1] : g->L.psi[1]);
+        case PHX_N: *bytes = cells * rb; return g->ws + (alt ? g->L.na[0] : g->L.n[0]);
+        case PHX_N_MINUS: *bytes = cells * rb; return g->ws + (alt ? g->L.na[1] : g->L.n[1]);
     }
     *bytes = 0;
     return nullptr;
 }
 
 void drop_graphs(phx_grid* g) {
-    if (g->g1) cudaGraphExecDestroy(g->g1);
+    for (int p = 0; p < 2; ++p) {
+        if (g->g1[p]) cudaGraphExecDestroy(g->g1[p]);
+        g->g1[p] = nullptr;
+    }
     if (g->gN) cudaGraphExecDestroy(g->gN);
-    g->g1 = g->gN = nullptr;
+    g->gN = nullptr;
     g->graphs_valid = false;
 }
 
 template <typename T>
-void fill_args(const phx_grid* g, StageArgs<T>& a) {
-    using C = typename Cx<T>::type;
-    std::memset(&a, 0, sizeof(a));
-    a.geo.nx = g->d.nx; a.geo.ny = g->d.ny; a.geo.batch = g->d.batch;
-    a.geo.bc_x = g->d.bc_x; a.geo.bc_y = g->d.bc_y;
-    a.geo.rows = g->rows;
-    a.geo.plane = plane_cells(g);
+void fill_geo_coef(const phx_grid* g, Geom& geo, Coef<T>& k) {
+    geo.nx = g->d.nx; geo.ny = g->d.ny; geo.batch = g->d.batch;
+    geo.bc_x = g->d.bc_x; geo.bc_y = g->d.bc_y;
+    geo.rows = g->rows;
+    geo.plane = plane_cells(g);
     const double* c = g->coef;
-    Coef<T>& k = a.k;
     k.cx = (T)c[0]; k.cy = (T)c[1]; k.ih = (T)c[2]; k.g = (T)c[3]; k.gx = (T)c[4]; k.gr = (T)c[5]; k.Rr = (T)c[6];
     k.hgc = (T)c[7]; k.gamr = (T)c[8]; k.bxx = (T)c[9]; k.byy = (T)c[10]; k.bxy = (T)c[11]; k.dt = (T)c[12];
     k.hdt = (T)(0.5 * c[12]);           // exact
@@ -161,6 +167,13 @@ void fill_args(const phx_grid* g, StageArgs<T>& a) {
     k.r13 = (T)(c[13] / (0.5 * c[12]));
     k.omega = c[17];
     k.dt_d = c[12];
+}
+
+template <typename T>
+void fill_args(const phx_grid* g, StageArgs<T>& a) {
+    using C = typename Cx<T>::type;
+    std::memset(&a, 0, sizeof(a));
+    fill_geo_coef<T>(g, a.geo, a.k);
     const int nc = model_spinor(g->d.model) ? 2 : 1;
     const bool res = model_reservoir(g->d.model);
     for (int s = 0; s < nc; ++s) {
@@ -218,18 +231,118 @@ cudaError_t enqueue_step_stage(phx_grid* g, cudaStream_t st) {
     return cudaSuccess;
 }
 
-int kernels_per_step(const phx_grid* g) { return g->variant == PHX_VARIANT_STAGE ? 4 : 4; }
+// ---- variant STEP: launch plan ---------------------------------------------------------------------------------
+int step_vec(const phx_grid* g) {
+    if (g->step_vec) return g->step_vec;
+    return (g->d.prec == PHX_C32 && g->d.nx % 2 == 0) ? 2 : 1;
+}
 
-cudaError_t enqueue_step(phx_grid* g, cudaStream_t st) {
+int step_occupancy(const phx_grid* g, int vec) {
+    const bool noise = g->d.noise != 0, zbc = g->d.bc_x || g->d.bc_y;
+    if (g->d.prec == PHX_C32) {
+        switch (g->d.model) {
+            case 0: return occupancy_step_32_0(noise, zbc, vec);
+            case 1: return occupancy_step_32_1(noise, zbc, vec);
+            case 2: return occupancy_step_32_2(noise, zbc, vec);
+            default: return occupancy_step_32_3(noise, zbc, vec);
+        }
+    }
+    switch (g->d.model) {
+        case 0: return occupancy_step_64_0(noise, zbc, vec);
+        case 1: return occupancy_step_64_1(noise, zbc, vec);
+        case 2: return occupancy_step_64_2(noise, zbc, vec);
+        default: return occupancy_step_64_3(noise, zbc, vec);
+    }
+}
+
+// Rows per chunk: every CTA costs (ly + 9) row iterations (4 + 4 halo rows and the pipeline fill), and the grid
+// runs in ceil(CTAs / resident CTAs) waves; pick the chunk count that minimises waves * (ly + 9).
+int step_rows_per_chunk(const phx_grid* g, int vec) {
+    if (g->step_ly) return g->step_ly < g->d.ny ? g->step_ly : g->d.ny;
+    const int strips = (g->d.nx + 32 * vec - 9) / (32 * vec - 8);
+    const long ctas_row = (long)((strips + 3) / 4) * g->d.batch;
+    const long slots = (long)g->n_sm * step_occupancy(g, vec);
+    long best_cost = -1;
+    int best_ly = g->d.ny;
+    const int max_chunks = g->d.ny / 8 > 0 ? g->d.ny / 8 : 1;
+    for (int nch = 1; nch <= max_chunks && nch <= 65535; ++nch) {
+        const int ly = (g->d.ny + nch - 1) / nch;
+        const int real_chunks = (g->d.ny + ly - 1) / ly;
+        const long waves = (ctas_row * real_chunks + slots - 1) / slots;
+        const long cost = waves * (ly + 9);
+        if (best_cost < 0 || cost < best_cost) { best_cost = cost; best_ly = ly; }
+    }
+    return best_ly;
+}
+
+// One RK4 step of variant STEP: a single kernel that reads the state of parity p and writes parity 1-p.
+template <typename T>
+cudaError_t enqueue_step_fused(phx_grid* g, cudaStream_t st, int parity) {
+    using C = typename Cx<T>::type;
+    StepArgs<T> a;
+    std::memset(&a, 0, sizeof(a));
+    fill_geo_coef<T>(g, a.geo, a.k);
+    const int nc = model_spinor(g->d.model) ? 2 : 1;
+    const bool res = model_reservoir(g->d.model);
+    for (int s = 0; s < nc; ++s) {
+        C* main_ = (C*)(g->ws + g->L.psi[s]);
+        C* alt = (C*)(g->ws + g->L.ya[s]);
+        a.psi_in[s] = parity ? alt : main_;
+        a.psi_out[s] = parity ? main_ : alt;
+        if (res) {
+            T* nmain = (T*)(g->ws + g->L.n[s]);
+            T* nalt = (T*)(g->ws + g->L.na[s]);
+            a.n_in[s] = parity ? nalt : nmain;
+            a.n_out[s] = parity ? nmain : nalt;
+        }
+    }
+    a.V = g->hasV ? (const T*)(g->ws + g->L.V) : nullptr;
+    a.P = g->hasP ? (const T*)(g->ws + g->L.P) : nullptr;
+    uint64_t* slots = (uint64_t*)(g->ws + g->L.step);
+    a.step_in = slots + parity;
+    a.step_out = slots + (1 - parity);
+    a.seed = g->prm.seed;
+    const int vec = step_vec(g);
+    a.strips = (g->d.nx + 32 * vec - 9) / (32 * vec - 8);
+    a.ly = step_rows_per_chunk(g, vec);
+    const dim3 grid((a.strips + 3) / 4, (g->d.ny + a.ly - 1) / a.ly, g->d.batch);
+    if (grid.y > 65535u) return cudaErrorInvalidConfiguration;
+    const bool noise = g->d.noise != 0, zbc = g->d.bc_x || g->d.bc_y;
+    if constexpr (sizeof(T) == 4) {
+        switch (g->d.model) {
+            case 0: return launch_step_32_0(a, noise, zbc, vec, grid, st);
+            case 1: return launch_step_32_1(a, noise, zbc, vec, grid, st);
+            case 2: return launch_step_32_2(a, noise, zbc, vec, grid, st);
+            default: return launch_step_32_3(a, noise, zbc, vec, grid, st);
+        }
+    } else {
+        switch (g->d.model) {
+            case 0: return launch_step_64_0(a, noise, zbc, vec, grid, st);
+            case 1: return launch_step_64_1(a, noise, zbc, vec, grid, st);
+            case 2: return launch_step_64_2(a, noise, zbc, vec, grid, st);
+            default: return launch_step_64_3(a, noise, zbc, vec, grid, st);
+        }
+    }
+}
+
+int kernels_per_step(const phx_grid* g) { return g->variant == PHX_VARIANT_STEP ? 1 : 4; }
+
+// Enqueues one step starting from state parity `parity` (always 0 for variant STAGE).
+cudaError_t enqueue_step(phx_grid* g, cudaStream_t st, int parity) {
+    if (g->variant == PHX_VARIANT_STEP)
+        return g->d.prec == PHX_C64 ? enqueue_step_fused<double>(g, st, parity) : enqueue_step_fused<float>(g, st, parity);
     return g->d.prec == PHX_C64 ? enqueue_step_stage<double>(g, st) : enqueue_step_stage<float>(g, st);
 }
 
-cudaError_t capture(phx_grid* g, int steps, cudaGraphExec_t* out) {
+cudaError_t capture(phx_grid* g, int steps, int parity, cudaGraphExec_t* out) {
     cudaGraph_t graph = nullptr;
     cudaError_t e = cudaStreamBeginCapture(g->cap_stream, cudaStreamCaptureModeThreadLocal);
     if (e != cudaSuccess) return e;
     cudaError_t le = cudaSuccess;
-    for (int s = 0; s < steps && le == cudaSuccess; ++s) le = enqueue_step(g, g->cap_stream);
+    for (int s = 0; s < steps && le == cudaSuccess; ++s) {
+        le = enqueue_step(g, g->cap_stream, parity);
+        if (g->variant == PHX_VARIANT_STEP) parity ^= 1;
+    }
     e = cudaStreamEndCapture(g->cap_stream, &graph);
     if (le != cudaSuccess) { if (graph) cudaGraphDestroy(graph); return le; }
     if (e != cudaSuccess) return e;
@@ -238,9 +351,38 @@ cudaError_t capture(phx_grid* g, int steps, cudaGraphExec_t* out) {
     return e;
 }
 
+bool step_variant_ok(const phx_grid* g) { return !g->hasE; }   // the fused step carries no drive term
+
 void resolve_variant(phx_grid* g) {
-    g->variant = PHX_VARIANT_STAGE;   // the only variant that runs every model / size
-    if (g->variant_req == PHX_VARIANT_STAGE) g->variant = PHX_VARIANT_STAGE;
+    if (g->variant_req == PHX_VARIANT_STEP && step_variant_ok(g)) g->variant = PHX_VARIANT_STEP;
+    else g->variant = PHX_VARIANT_STAGE;   // runs every model, size and term
+}
+
+// Variant STAGE keeps the state in psi/n: if the fused-step ping-pong left it in the alternate buffers, move it
+// back (and realign the device step-counter slots) before another variant runs.
+phx_status normalise_state(phx_grid* g) {
+    if (g->parity == 0) return PHX_OK;
+    const int nc = model_spinor(g->d.model) ? 2 : 1;
+    const size_t cells = plane_cells(g) * g->d.batch, rb = real_bytes(g);
+    for (int s = 0; s < nc; ++s) {
+        PHX_CUDA(g, cudaMemcpyAsync(g->ws + g->L.psi[s], g->ws + g->L.ya[s], cells * 2 * rb, cudaMemcpyDeviceToDevice, g->stream));
+        if (model_reservoir(g->d.model))
+            PHX_CUDA(g, cudaMemcpyAsync(g->ws + g->L.n[s], g->ws + g->L.na[s], cells * rb, cudaMemcpyDeviceToDevice, g->stream));
+    }
+    const uint64_t slots[2] = {g->step_host, g->step_host};
+    PHX_CUDA(g, cudaMemcpyAsync(g->ws + g->L.step, slots, sizeof(slots), cudaMemcpyHostToDevice, g->stream));
+    PHX_CUDA(g, cudaStreamSynchronize(g->stream));
+    g->parity = 0;
+    return PHX_OK;
+}
+
+// Re-resolves the variant after a request or a change of the terms present; drops the captured graphs.
+phx_status apply_variant(phx_grid* g) {
+    const int before = g->variant;
+    resolve_variant(g);
+    drop_graphs(g);
+    if (before == PHX_VARIANT_STEP && g->variant != PHX_VARIANT_STEP) return normalise_state(g);
+    return PHX_OK;
 }
 
 phx_status copy_in(phx_grid* g, void* dst, const void* src, size_t bytes, phx_mem where) {
@@ -303,10 +445,14 @@ phx_status phx_create_grid(phx_grid** out, const phx_grid_desc* desc) {
     g->variant_req = PHX_VARIANT_AUTO;
     g->rows = 16;
     g->vec = (desc->prec == PHX_C32 && desc->nx % 2 == 0) ? 2 : 1;
-    g->graph_steps = 8;
-    g->g1 = g->gN = nullptr;
+    g->graph_steps = g->gsteps = 8;
+    g->g1[0] = g->g1[1] = g->gN = nullptr;
     g->graphs_valid = false;
+    g->parity = 0;
+    g->step_ly = g->step_vec = 0;
+    g->n_sm = prop.multiProcessorCount;
     g->sticky = cudaSuccess;
+    g->variant = PHX_VARIANT_STAGE;
     resolve_variant(g);
     if (cudaStreamCreateWithFlags(&g->cap_stream, cudaStreamNonBlocking) != cudaSuccess) { delete g; return PHX_ERR_CUDA; }
     // zero the state, the static fields and the step counter
@@ -372,8 +518,9 @@ phx_status phx_set_drive(phx_grid* g, const void* E, phx_mem where) {
     if (!g || (where != PHX_HOST && where != PHX_DEVICE)) return PHX_ERR_INVALID_ARG;
     if (g->sticky != cudaSuccess) return PHX_ERR_CUDA;
     if (E) { phx_status s = copy_in(g, g->ws + g->L.E, E, plane_cells(g) * 2 * real_bytes(g), where); if (s) return s; }
-    if (g->hasE != (E != nullptr)) drop_graphs(g);
+    const bool changed = g->hasE != (E != nullptr);
     g->hasE = E != nullptr;
+    if (changed) return apply_variant(g);
     return PHX_OK;
 }
 
@@ -402,17 +549,27 @@ phx_status phx_step_rk4(phx_grid* g, int64_t n_steps) {
     if (n_steps == 0) return PHX_OK;
     if (!g->graphs_valid) {
         drop_graphs(g);
-        PHX_CUDA(g, capture(g, 1, &g->g1));
-        PHX_CUDA(g, capture(g, g->graph_steps, &g->gN));
+        PHX_CUDA(g, capture(g, 1, 0, &g->g1[0]));
+        if (g->variant == PHX_VARIANT_STEP) PHX_CUDA(g, capture(g, 1, 1, &g->g1[1]));
+        // the multi-step graph of the ping-pong variant must return to parity 0: an even number of steps
+        g->gsteps = g->variant == PHX_VARIANT_STEP ? (g->graph_steps < 2 ? 2 : g->graph_steps & ~1) : g->graph_steps;
+        PHX_CUDA(g, capture(g, g->gsteps, 0, &g->gN));
         g->graphs_valid = true;
     }
+    const bool pingpong = g->variant == PHX_VARIANT_STEP;
     int64_t left = n_steps;
-    while (left >= g->graph_steps) {
+    if (pingpong && g->parity == 1) {   // the multi-step graph is captured from parity 0
+        PHX_CUDA(g, cudaGraphLaunch(g->g1[1], g->stream));
+        g->parity = 0;
+        --left;
+    }
+    while (left >= g->gsteps) {
         PHX_CUDA(g, cudaGraphLaunch(g->gN, g->stream));
-        left -= g->graph_steps;
+        left -= g->gsteps;
     }
     while (left > 0) {
-        PHX_CUDA(g, cudaGraphLaunch(g->g1, g->stream));
+        PHX_CUDA(g, cudaGraphLaunch(g->g1[pingpong ? g->parity : 0], g->stream));
+        if (pingpong) g->parity ^= 1;
         --left;
     }
     g->step_host += (uint64_t)n_steps;
@@ -443,7 +600,7 @@ phx_status phx_ensemble_mean_density(phx_grid* g, phx_field f, void* dst, phx_me
     if (!field_present(g, f)) return fail(g, PHX_ERR_UNSUPPORTED, "phx_ensemble_mean_density: field not present");
     size_t bytes;
     void* psi = field_ptr(g, f, &bytes);
-    void* scratch = g->ws + g->L.ya[0];   // stage buffers are dead between steps
+    void* scratch = g->ws + g->L.yb[0];   // dead between steps in every variant
     PHX_CUDA(g, launch_ensemble_mean(psi, scratch, g->d.prec == PHX_C64, plane_cells(g), g->d.batch, g->stream));
     g->launches += 1;
     return copy_out(g, dst, scratch, plane_cells(g) * real_bytes(g), where);
@@ -466,11 +623,11 @@ phx_status phx_debug_noise_u32(phx_grid* g, uint64_t step, uint32_t* dst, phx_me
         PHX_CUDA(g, cudaStreamSynchronize(g->stream));
         return PHX_OK;
     }
-    // stage through the (dead between steps) stage buffers, one chunk of realisations at a time
+    // stage through the buffers that are dead between steps (yb, acc), one chunk of realisations at a time
     const size_t per_real = plane * 16;
     const size_t chunk = g->L.scratch_bytes / per_real;
     if (chunk < 1) return fail(g, PHX_ERR_UNSUPPORTED, "phx_debug_noise_u32: scratch too small");
-    uint32_t* scratch = (uint32_t*)(g->ws + g->L.ya[0]);
+    uint32_t* scratch = (uint32_t*)(g->ws + g->L.yb[0]);
     for (size_t r0 = 0; r0 < (size_t)g->d.batch; r0 += chunk) {
         const size_t nr = (size_t)g->d.batch - r0 < chunk ? (size_t)g->d.batch - r0 : chunk;
         PHX_CUDA(g, launch_noise_words(scratch, g->prm.seed, step, plane, (int)r0, (int)nr, g->stream));
@@ -482,12 +639,11 @@ phx_status phx_debug_noise_u32(phx_grid* g, uint64_t step, uint32_t* dst, phx_me
 
 phx_status phx_select_variant(phx_grid* g, int32_t variant) {
     if (!g) return PHX_ERR_INVALID_ARG;
-    if (variant != PHX_VARIANT_AUTO && variant != PHX_VARIANT_STAGE)
+    if (g->sticky != cudaSuccess) return PHX_ERR_CUDA;
+    if (variant != PHX_VARIANT_AUTO && variant != PHX_VARIANT_STAGE && !(variant == PHX_VARIANT_STEP && step_variant_ok(g)))
         return fail(g, PHX_ERR_UNSUPPORTED, "phx_select_variant: variant not available for this grid/model");
     g->variant_req = variant;
-    resolve_variant(g);
-    drop_graphs(g);
-    return PHX_OK;
+    return apply_variant(g);
 }
 
 phx_status phx_get_variant(const phx_grid* g, int32_t* variant) {
@@ -511,6 +667,13 @@ phx_status phx_set_tuning(phx_grid* g, const char* key, int32_t value) {
         if (value != 1 && value != 2) return PHX_ERR_INVALID_ARG;
         if (value == 2 && g->d.nx % 2 != 0) return fail(g, PHX_ERR_UNSUPPORTED, "vec=2 needs even nx");
         g->vec = value;
+    } else if (!std::strcmp(key, "step_ly")) {        // variant STEP: rows per chunk (0 = automatic)
+        if (value < 0 || value > (1 << 20)) return PHX_ERR_INVALID_ARG;
+        g->step_ly = value;
+    } else if (!std::strcmp(key, "step_vec")) {       // variant STEP: cells per lane (0 = automatic)
+        if (value < 0 || value > 2) return PHX_ERR_INVALID_ARG;
+        if (value == 2 && (g->d.nx % 2 != 0 || g->d.prec != PHX_C32)) return fail(g, PHX_ERR_UNSUPPORTED, "step_vec=2 needs complex fp32 and even nx");
+        g->step_vec = value;
     } else if (!std::strcmp(key, "graph_steps")) {
         if (value < 1 || value > 256) return PHX_ERR_INVALID_ARG;
         g->graph_steps = value;

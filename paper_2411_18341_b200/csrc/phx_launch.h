@@ -16,6 +16,21 @@ PHX_DECL_STAGE(32, float)
 PHX_DECL_STAGE(64, double)
 #undef PHX_DECL_STAGE
 
+template <typename T> struct StepArgs;
+
+#define PHX_DECL_STEP(P, T)                                                                                      \
+    cudaError_t launch_step_##P##_0(const StepArgs<T>&, bool noise, bool zbc, int vec, dim3 grid, cudaStream_t); \
+    cudaError_t launch_step_##P##_1(const StepArgs<T>&, bool noise, bool zbc, int vec, dim3 grid, cudaStream_t); \
+    cudaError_t launch_step_##P##_2(const StepArgs<T>&, bool noise, bool zbc, int vec, dim3 grid, cudaStream_t); \
+    cudaError_t launch_step_##P##_3(const StepArgs<T>&, bool noise, bool zbc, int vec, dim3 grid, cudaStream_t); \
+    int occupancy_step_##P##_0(bool noise, bool zbc, int vec);                                                    \
+    int occupancy_step_##P##_1(bool noise, bool zbc, int vec);                                                    \
+    int occupancy_step_##P##_2(bool noise, bool zbc, int vec);                                                    \
+    int occupancy_step_##P##_3(bool noise, bool zbc, int vec);
+PHX_DECL_STEP(32, float)
+PHX_DECL_STEP(64, double)
+#undef PHX_DECL_STEP
+
 // phx_aux.cu: small helper kernels
 cudaError_t launch_ensemble_mean(const void* psi, void* out, int prec64, size_t plane, int batch, cudaStream_t);
 cudaError_t launch_noise_words(uint32_t* out, uint32_t seed, uint64_t step, size_t plane, int r0, int batch, cudaStream_t);

@@ -1,0 +1,212 @@
+"""GPU parity of variant STEP (one kernel per RK4 step, four stages temporally blocked in registers; DESIGN.md
+section 5.2) against the CPU oracle, element by element, plus the invariants that need no oracle.
+Bars as in test_gpu_parity.py (BASELINE.json north_star): relative L2 <= 1e-12 (complex fp64), <= 2e-5 (complex fp32).
+Sizes span several warp strips (56 / 24 output columns per strip) and row chunks with ragged tails in x and y."""
+import numpy as np
+import pytest
+
+from paper_2411_18341_b200 import workloads as wl
+from helpers import TOL, compare, make_gpu, make_oracle, rel_l2
+
+pytestmark = pytest.mark.gpu
+STEP, STAGE = 3, 1
+
+
+def run_pair(w, n_steps, tuning=None, **kw):
+    g = make_gpu(w, variant=STEP, tuning=tuning, **kw)
+    assert g.get_variant() == STEP
+    o = make_oracle(w, **{k: v for k, v in kw.items() if k in ("bc", "E", "extra_params")})
+    g.step_rk4(n_steps)
+    o.step_rk4(n_steps)
+    errs = compare(g, o, w)
+    assert g.get_launch_count() == n_steps        # one kernel per RK4 step
+    g.destroy()
+    return errs
+
+
+def test_cfg1_full_run_fp64():
+    w = wl.cfg1()
+    errs = run_pair(w, w.n_steps)
+    assert errs["psi_p"] <= 1e-12
+
+
+@pytest.mark.parametrize("prec", ["c32", "c64"])
+@pytest.mark.parametrize("nx,ny", [(600, 75), (514, 40), (201, 67), (64, 64), (56, 9), (8, 5)])
+def test_cfg2_reduced(prec, nx, ny):
+    # odd nx runs one cell per lane; nx < strip width wraps a strip onto itself
+    w = wl.cfg2(n=nx, ny=ny, prec=prec)
+    run_pair(w, 101)                               # odd count: the state ends in the alternate buffer
+
+
+@pytest.mark.parametrize("tuning", [{"step_ly": 8}, {"step_ly": 13, "step_vec": 1}, {"step_ly": 1000}])
+def test_cfg2_chunking(tuning):
+    w = wl.cfg2(n=300, ny=70, prec="c32")
+    run_pair(w, 60, tuning=tuning)
+
+
+@pytest.mark.parametrize("prec", ["c32", "c64"])
+def test_cfg2_1024_horizon(prec):
+    w = wl.cfg2(n=1024, prec=prec)
+    run_pair(w, 40)
+
+
+@pytest.mark.parametrize("prec", ["c32", "c64"])
+@pytest.mark.parametrize("n", [96, 300])
+def test_cfg3_reservoir_reduced(prec, n):
+    w = wl.cfg3(n=n, prec=prec)
+    run_pair(w, 200)
+
+
+@pytest.mark.parametrize("prec", ["c32", "c64"])
+def test_cfg4_spinor_reduced(prec):
+    w = wl.cfg4(n=320, prec=prec, sigma_cells=20.0)
+    run_pair(w, 100)
+
+
+@pytest.mark.parametrize("prec", ["c32", "c64"])
+def test_spinor_reservoir_example3(prec):
+    w = wl.example3(n=150, prec=prec)
+    run_pair(w, 100)
+
+
+@pytest.mark.parametrize("bc", [(1, 1), (1, 0), (0, 1)])
+@pytest.mark.parametrize("model", ["scalar", "spinor_reservoir"])
+def test_zero_boundaries(bc, model):
+    w = wl.cfg2(n=130, ny=70, prec="c64") if model == "scalar" else wl.example3(n=90, prec="c64")
+    run_pair(w, 50, bc=bc)
+
+
+def test_zero_boundaries_fp32_two_cells_per_lane():
+    w = wl.cfg2(n=130, ny=70, prec="c32")
+    run_pair(w, 50, bc=(1, 1), tuning={"step_ly": 16})
+
+
+def test_density_offset():
+    w = wl.cfg2(n=128, ny=64, prec="c64")
+    run_pair(w, 50, extra_params=dict(density_offset=0.02))
+
+
+def test_drive_is_not_available_in_the_fused_step():
+    from paper_2411_18341_b200 import binding as phx
+    w = wl.cfg2(n=64, ny=32, prec="c32")
+    E = np.zeros((w.ny, w.nx), np.complex64)
+    g = make_gpu(w, E=E)
+    with pytest.raises(phx.PhxError) as e:
+        g.select_variant(STEP)
+    assert e.value.status == phx.PHX_ERR_UNSUPPORTED
+    g.destroy()
+    g = make_gpu(w, variant=STEP)
+    g.step_rk4(3)                                  # odd: state in the alternate buffer
+    g.set_drive(E)                                 # falls back to STAGE and moves the state back
+    assert g.get_variant() == STAGE
+    g.step_rk4(2)
+    o = make_oracle(w, E=E)
+    o.step_rk4(5)
+    compare(g, o, w)
+    g.destroy()
+
+
+# ---- stochastic path -------------------------------------------------------------------------------------
+@pytest.mark.parametrize("prec", ["c32", "c64"])
+def test_cfg5_noisy_ensemble_reduced(prec):
+    w = wl.cfg5(n=64, batch=6, prec=prec)
+    g = make_gpu(w, variant=STEP)
+    o = make_oracle(w)
+    g.step_rk4(61)
+    o.step_rk4(61)
+    compare(g, o, w)
+    mean = g.ensemble_mean_density("psi_p")
+    assert rel_l2(mean, o.ensemble_mean_density("psi_p")) <= TOL[prec]
+    g.destroy()
+
+
+def test_noise_one_step_from_zero_matches_normal_map():
+    w = wl.cfg5(n=64, batch=3, prec="c32")
+    w.fields["psi_p"][...] = 0
+    g = make_gpu(w, variant=STEP)
+    o = make_oracle(w)
+    g.step_rk4(1)
+    o.step_rk4(1)
+    got = g.read_field("psi_p")
+    assert np.max(np.abs(got - o.psi_p)) <= 4e-7 * np.max(np.abs(o.psi_p))
+    g.destroy()
+
+
+def test_spinor_noise():
+    w = wl.cfg4(n=96, prec="c32", sigma_cells=10.0)
+    w.noise, w.seed = True, 11
+    run_pair(w, 30)
+
+
+# ---- invariants (no oracle) --------------------------------------------------------------------------------
+@pytest.mark.parametrize("model", ["scalar", "reservoir", "spinor", "spinor_reservoir"])
+def test_shift_equivariance_bit_exact(model):
+    maker = {"scalar": lambda: wl.cfg2(n=300, ny=70, prec="c32"), "reservoir": lambda: wl.cfg3(n=200, prec="c32"),
+             "spinor": lambda: wl.cfg4(n=200, prec="c32", sigma_cells=15.0), "spinor_reservoir": lambda: wl.example3(n=140)}[model]
+    w = maker()
+    g = make_gpu(w, variant=STEP)
+    g.step_rk4(10)
+    base = {k: g.read_field(k) for k in w.fields}
+    g.destroy()
+    sh = (37, -5)   # every cell is computed by the same instruction sequence whatever its lane, strip or chunk
+    w2 = maker()
+    for k in w2.fields:
+        w2.fields[k] = np.ascontiguousarray(np.roll(w2.fields[k], sh, (1, 2)))
+    if w2.V is not None:
+        w2.V = np.ascontiguousarray(np.roll(w2.V, sh, (0, 1)))
+    if w2.P is not None:
+        w2.P = np.ascontiguousarray(np.roll(w2.P, sh, (0, 1)))
+    g2 = make_gpu(w2, variant=STEP, tuning={"step_ly": 19})
+    g2.step_rk4(10)
+    for k in w.fields:
+        assert np.array_equal(np.roll(base[k], sh, (1, 2)), g2.read_field(k)), k
+    g2.destroy()
+
+
+def test_step_splitting_and_checkpoint_are_bit_exact_with_noise():
+    w = wl.cfg5(n=64, batch=3)
+    g1, g2 = make_gpu(w, variant=STEP), make_gpu(w, variant=STEP)
+    g1.step_rk4(23)
+    for n in (1, 8, 9, 5):
+        g2.step_rk4(n)
+    assert g1.get_step() == g2.get_step() == 23
+    for k in w.fields:
+        assert np.array_equal(g1.read_field(k), g2.read_field(k))
+    # checkpoint at an odd step, restart in a fresh handle
+    snap = {k: g1.read_field(k) for k in w.fields}
+    g1.step_rk4(6)
+    g3 = make_gpu(w, variant=STEP)
+    for k, v in snap.items():
+        g3.set_field(k, v)
+    g3.set_step(23)
+    g3.step_rk4(6)
+    for k in w.fields:
+        assert np.array_equal(g1.read_field(k), g3.read_field(k))
+    for g in (g1, g2, g3):
+        g.destroy()
+
+
+def test_switching_variants_mid_run_keeps_state_and_noise_stream():
+    w = wl.cfg5(n=64, batch=2)
+    g = make_gpu(w, variant=STEP)
+    g.step_rk4(5)
+    g.select_variant(STAGE)
+    g.step_rk4(4)
+    g.select_variant(STEP)
+    g.step_rk4(3)
+    o = make_oracle(w)
+    o.step_rk4(12)
+    compare(g, o, w)
+    assert g.get_step() == 12
+    g.destroy()
+
+
+def test_step_and_stage_agree_to_rounding():
+    w = wl.cfg3(n=192, prec="c64")
+    a, b = make_gpu(w, variant=STEP), make_gpu(w, variant=STAGE)
+    a.step_rk4(50)
+    b.step_rk4(50)
+    for k in w.fields:
+        assert rel_l2(a.read_field(k), b.read_field(k)) <= 1e-13
+    a.destroy()
+    b.destroy()

@@ -22,6 +22,13 @@
 #include "phx_deriv.cuh"
 #include "phx_philox.cuh"
 
+#ifndef PHX_STEP_UNROLL
+#define PHX_STEP_UNROLL 4
+#endif
+#ifndef PHX_STEP_PF_ROWS
+#define PHX_STEP_PF_ROWS 6
+#endif
+
 namespace phx {
 
 template <typename T>
@@ -76,6 +83,9 @@ template <int VEC> __device__ __forceinline__ void str(double* p, const double (
     if constexpr (VEC == 2) *reinterpret_cast<double2*>(p) = make_double2(v[0], v[1]);
     else *p = v[0];
 }
+
+// DRAM -> L2 prefetch of the line holding p (no register is tied up; the register fetch one row ahead then hits L2).
+__device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
 
 __device__ __forceinline__ float2 up1(float2 v) { return make_float2(__shfl_up_sync(0xffffffffu, v.x, 1), __shfl_up_sync(0xffffffffu, v.y, 1)); }
 __device__ __forceinline__ float2 dn1(float2 v) { return make_float2(__shfl_down_sync(0xffffffffu, v.x, 1), __shfl_down_sync(0xffffffffu, v.y, 1)); }
@@ -188,9 +198,47 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
     if (!zy) { qw %= ny; if (qw < 0) qw += ny; }
     int qprev = 0;          // wrapped index of the row fetched in the previous iteration (= row j+1 now)
     bool okprev = false;
+    // rows further ahead are pulled from DRAM into L2 by prefetch instructions (PF_ROWS ahead of the register fetch)
+    constexpr int PF_ROWS = PHX_STEP_PF_ROWS;
+    constexpr int UNROLL_J = PHX_STEP_UNROLL;
+    int qpf = r0 - 4 + PF_ROWS;
+    if (!zy) { qpf %= ny; if (qpf < 0) qpf += ny; }
+    if (PF_ROWS > 0 && inx) {
+        // warm-up: the first PF_ROWS rows of the chunk
+        int q = r0 - 4;
+        if (!zy) { q %= ny; if (q < 0) q += ny; }
+        for (int r = 0; r < PF_ROWS; ++r) {
+            if (!zy || (q >= 0 && q < ny)) {
+                const size_t o = (size_t)q * nx + xg;
+#pragma unroll
+                for (int s = 0; s < NC; ++s) {
+                    prefetch_l2(a.psi_in[s] + boff + o);
+                    if (RES) prefetch_l2(a.n_in[s] + boff + o);
+                }
+                if (a.V) prefetch_l2(a.V + o);
+                if (RES && a.P) prefetch_l2(a.P + o);
+            }
+            ++q;
+            if (!zy && q == ny) q = 0;
+        }
+    }
 
-#pragma unroll 1
+#pragma unroll UNROLL_J
     for (int j = r0 - 6; j <= r1 + 2; ++j) {
+        if (PF_ROWS > 0) {
+            if (inx && (j + 2 + PF_ROWS <= r1 + 3) && (!zy || (qpf >= 0 && qpf < ny))) {
+                const size_t o = (size_t)qpf * nx + xg;
+#pragma unroll
+                for (int s = 0; s < NC; ++s) {
+                    prefetch_l2(a.psi_in[s] + boff + o);
+                    if (RES) prefetch_l2(a.n_in[s] + boff + o);
+                }
+                if (a.V) prefetch_l2(a.V + o);
+                if (RES && a.P) prefetch_l2(a.P + o);
+            }
+            ++qpf;
+            if (!zy && qpf == ny) qpf = 0;
+        }
         // ---- fetch: psi row j+2; row-local inputs (V, P, n) of row j+1 -----------------------------------------------
         const bool okq = inx && (j + 2 <= r1 + 3) && (!zy || (qw >= 0 && qw < ny));
         {

@@ -74,6 +74,22 @@ def algo_bytes_per_cell_step(w, variant):
     return b
 
 
+def algo_flops_per_cell_step(w):
+    """Floating-point operations the method itself asks for per cell-step (counted from the
+    formulas of section 2, an FMA = 2): per stage and component the derivative costs 33 (Laplacian 18, density 4,
+    potential 3, K 8), +9 with a reservoir (g_r n 2, gain 3, K_n 4), +36 in a spinor (cross density 6, TE-TM 30);
+    the fused RK sums cost 28 per component (+14 per reservoir).  The Philox/Box-Muller work of the noise is not counted."""
+    ncomp = 2 if w.model.startswith("spinor") else 1
+    res = w.model.endswith("reservoir")
+    per_stage = 33 + (9 if res else 0) + (36 if ncomp == 2 else 0)
+    return ncomp * (4 * per_stage + 28 + (14 if res else 0))
+
+
+# Plain-ALU peak (no tensor cores: the stencil is not a contraction): 148 SMs x 128 FP32 (64 FP64) lanes x 2 flop x
+# 1.965 GHz (B200_PROFILING.md unit counts and clocks.max.sm); DESIGN.md section 6.
+ALU_PEAK_TFLOPS = {"c32": 148 * 128 * 2 * 1.965e9 / 1e12, "c64": 148 * 64 * 2 * 1.965e9 / 1e12}
+
+
 class ClockSampler:
     """Samples nvidia-smi clocks and throttle reasons while the timed region runs."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
@@ -183,6 +199,7 @@ def main():
     ap.add_argument("--tune", default="", help="comma separated key=value passed to phx_set_tuning")
     ap.add_argument("--e2e-steps", type=int, default=20)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-stage-leg", action="store_true", help="skip the extra timing of variant STAGE")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
@@ -217,30 +234,51 @@ def main():
             torch.cuda.synchronize()
 
     # ---- device-resident throughput ---------------------------------------------------------------------
+    def timed(steps):
+        """CUDA events on the launching stream around `steps` RK4 steps, barrier + synchronize on both sides."""
+        launches0 = g.get_launch_count()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        e0.record(stream)
+        g.step_rk4(steps)
+        e1.record(stream)
+        barrier()
+        t_ms = e0.elapsed_time(e1)
+        if world > 1:
+            t = torch.tensor([t_ms], device="cuda")
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            t_ms = float(t.item())
+        return t_ms, g.get_launch_count() - launches0
+
     g.step_rk4(args.warmup)
     barrier()
     sampler = ClockSampler(local)
     if rank == 0:
         sampler.start()
         time.sleep(0.25)
-    launches0 = g.get_launch_count()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    barrier()
     t_wall0 = time.time()
-    e0.record(stream)
-    g.step_rk4(args.steps)
-    e1.record(stream)
-    barrier()
+    ms, launches = timed(args.steps)
     t_wall1 = time.time()
-    ms = e0.elapsed_time(e1)
-    launches = g.get_launch_count() - launches0
     clocks = sampler.stop(t_wall0, t_wall1) if rank == 0 else None
-    if world > 1:
-        t = torch.tensor([ms], device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
     cells = w.cells
     value = world * cells * args.steps / (ms * 1e-3) / 1e9
+
+    # the per-stage variant (the HBM-bound kernels of the north_star's >= 70 % target), timed the same way on a
+    # shorter run, when the headline ran the fused step
+    stage_info = None
+    if variant != phx.PHX_VARIANT_STAGE and not args.no_stage_leg:
+        g.select_variant(phx.PHX_VARIANT_STAGE)
+        g.step_rk4(args.warmup)
+        st_steps = max(8, args.steps // 4)
+        st_ms, st_launches = timed(st_steps)
+        st_bpc = algo_bytes_per_cell_step(w, phx.PHX_VARIANT_STAGE)
+        st_val = world * cells * st_steps / (st_ms * 1e-3) / 1e9
+        st_gbs = st_bpc * cells * st_steps / (st_ms * 1e-3) / 1e9
+        stage_info = {"variant": 1, "kernel": "phx::stage_kernel (4 launches per step)", "value": st_val, "unit": UNIT,
+                      "steps": st_steps, "ms_per_step": st_ms / st_steps, "gpu_launches": int(st_launches),
+                      "algorithmic_bytes_per_cell_step": st_bpc,
+                      "roofline": {"bound": "hbm", "achieved": st_gbs, "unit": "GB/s"}}
+        g.select_variant(variant)
     finite = bool(np.all(np.isfinite(g.read_field("psi_p")[0, :4])))
 
     # ---- end to end through the C ABI with host buffers ----------------------------------------------------
@@ -282,18 +320,32 @@ def main():
     launch_ms = ms / launches
     achieved = bytes_per_launch / (launch_ms * 1e-3) / 1e9
     comp = COMPULSORY_BYTES[w.model] * (2 if w.prec == "c64" else 1)
-    roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": None, "peak_source": peak_src, "kernel": {1: "phx::stage_kernel (4 launches per step)", 3: "phx::step_kernel (1 launch per step)"}.get(variant, str(variant)),
-                "algorithmic_bytes_per_cell_step": bpc, "bytes_per_launch": bytes_per_launch,
-                "avg_launch_ms": launch_ms, "compulsory_bytes_per_cell_step": comp,
-                "compulsory_frac": value / world * 1e9 * comp / 1e9 / peak}
-    traffic_file = os.path.join(ROOT, "profiles", "traffic.json")
+    kernel = {1: "phx::stage_kernel (4 launches per step)", 3: "phx::step_kernel (1 launch per step)"}.get(variant, str(variant))
+    hbm = {"achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "peak_source": peak_src,
+           "algorithmic_bytes_per_cell_step": bpc, "bytes_per_launch": bytes_per_launch,
+           "compulsory_bytes_per_cell_step": comp, "compulsory_frac": value / world * 1e9 * comp / 1e9 / peak}
+    if variant == phx.PHX_VARIANT_STEP:
+        # the fused step moves the compulsory bytes only; it is bound by plain FP32/FP64 instruction issue
+        fpc = algo_flops_per_cell_step(w)
+        alu_peak = ALU_PEAK_TFLOPS[w.prec]
+        tf = fpc * cells / kernels_per_step / (launch_ms * 1e-3) / 1e12
+        roofline = {"bound": "alu", "achieved": tf, "peak": alu_peak, "unit": "TFLOP/s", "frac": tf / alu_peak,
+                    "traffic": None, "peak_source": "derived: 148 SM x 128 (fp64: 64) lanes x 2 x 1.965 GHz, no tensor cores",
+                    "kernel": kernel, "algorithmic_flops_per_cell_step": fpc, "flops_per_launch": fpc * cells / kernels_per_step,
+                    "avg_launch_ms": launch_ms, "hbm": hbm}
+    else:
+        roofline = dict(hbm, bound="hbm", traffic=None, kernel=kernel, avg_launch_ms=launch_ms)
+    if stage_info is not None:
+        stage_info["roofline"].update(peak=peak, frac=stage_info["roofline"]["achieved"] / peak, peak_source=peak_src)
+    # DRAM bytes per launch of this kernel from the committed `ncu --set full` capture (profiles/traffic.csv)
+    traffic_file = os.path.join(ROOT, "profiles", "traffic.csv")
     if os.path.exists(traffic_file):
         try:
-            tr = json.load(open(traffic_file)).get(f"{args.workload}:v{variant}")
-            if tr:
-                roofline["traffic"] = tr["dram_bytes_per_launch"]
-                roofline["traffic_source"] = tr["source"]
+            for line in open(traffic_file):
+                p = [x.strip() for x in line.split(",")]
+                if len(p) >= 4 and p[0] == args.workload and p[1] == str(variant):
+                    roofline["traffic"] = float(p[2])
+                    roofline["traffic_source"] = p[3]
         except Exception:
             pass
 
@@ -324,7 +376,7 @@ def main():
         "clocks": clocks, "gpu_launches": int(launches),
         "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                 "rk4_steps_per_call": 1, "steps": args.e2e_steps},
-        "roofline": roofline, "cpu_baseline": cpu,
+        "roofline": roofline, "cpu_baseline": cpu, "stage_variant": stage_info,
     }
     del out["config"]["model"]
     print(json.dumps(out))

@@ -61,9 +61,10 @@ typedef enum { PHX_BC_PERIODIC = 0, PHX_BC_ZERO = 1 } phx_boundary;   /* PAPER.m
 
 /* Kernel variants (all compute the same RK4 step; they differ in how often data crosses HBM). */
 typedef enum {
-    PHX_VARIANT_AUTO = 0,
-    PHX_VARIANT_STAGE = 1,     /* one fused kernel per RK stage (4 launches per step) */
-    PHX_VARIANT_STEP = 3,      /* one kernel per RK4 step, four stages on a haloed tile in shared memory */
+    PHX_VARIANT_AUTO = 0,      /* the fastest variant that can run the grid: STEP, or STAGE when a drive is set */
+    PHX_VARIANT_STAGE = 1,     /* one fused kernel per RK stage (4 launches per step); every model and term */
+    PHX_VARIANT_STEP = 3,      /* one kernel per RK4 step: the four stages pipelined along y in register windows of
+                                  a haloed warp-wide column strip (N_halo = 4); no drive term */
     PHX_VARIANT_RESIDENT = 4   /* whole grid resident on chip, many steps per launch (small grids) */
 } phx_variant;
 
@@ -141,11 +142,14 @@ phx_status phx_get_coeffs(const phx_grid* g, double* out, int32_t n);
  * dst[batch][ny][nx][4], produced by the same device function the stepping kernels call. */
 phx_status phx_debug_noise_u32(phx_grid* g, uint64_t step, uint32_t* dst, phx_mem where);
 
-/* Selects a kernel variant (phx_variant).  UNSUPPORTED if it cannot run this grid/model. */
+/* Selects a kernel variant (phx_variant).  UNSUPPORTED if it cannot run this grid/model.  All variants
+ * compute the same RK4 step (results agree to rounding); the state and the step counter carry over. */
 phx_status phx_select_variant(phx_grid* g, int32_t variant);
 
 /* Bench/test aids: the variant the next phx_step_rk4 will use; kernels launched so far by this handle;
- * launch geometry knobs (key/value, UNSUPPORTED for unknown keys). */
+ * launch geometry knobs (key/value, UNSUPPORTED for unknown keys): "rows", "vec" (variant STAGE: rows per
+ * CTA, cells per thread), "step_ly", "step_vec" (variant STEP: rows per chunk, cells per lane; 0 = automatic),
+ * "graph_steps" (RK4 steps per captured CUDA graph).  Results do not depend on them. */
 phx_status phx_get_variant(const phx_grid* g, int32_t* variant);
 phx_status phx_get_launch_count(const phx_grid* g, uint64_t* launches);
 phx_status phx_set_tuning(phx_grid* g, const char* key, int32_t value);

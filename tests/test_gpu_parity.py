@@ -1,13 +1,18 @@
-"""GPU parity: libphx (CUDA, through the C ABI) against the CPU oracle, element by element, on the same
+"""GPU parity of variant STAGE (one fused kernel per RK stage): libphx (CUDA, through the C ABI) against the CPU oracle, element by element, on the same
 seeded inputs.  Bars (BASELINE.json north_star): relative L2 <= 1e-12 (complex fp64), <= 2e-5 (complex fp32);
 Philox words bit-exact.  Sizes span several tiles plus a ragged tail (block tile: 256 x rows cells)."""
 import numpy as np
 import pytest
 
 from paper_2411_18341_b200 import workloads as wl
-from helpers import TOL, compare, make_gpu, make_oracle, rel_l2
+import functools
+
+import helpers
+from helpers import TOL, compare, make_oracle, rel_l2
 
 pytestmark = pytest.mark.gpu
+STAGE = 1
+make_gpu = functools.partial(helpers.make_gpu, variant=STAGE)   # AUTO resolves to the fused step (test_gpu_step_variant.py)
 
 
 def run_pair(w, n_steps, **kw):
@@ -196,6 +201,7 @@ def test_device_buffers_and_api_errors():
     from paper_2411_18341_b200 import binding as phx
     w = wl.cfg2(n=128, ny=64, prec="c32")
     g = phx.Grid(w.nx, w.ny, w.dx, w.dy)
+    g.select_variant(STAGE)
     with pytest.raises(phx.PhxError) as e:
         g.step_rk4(1)
     assert e.value.status == phx.PHX_ERR_BAD_STATE

@@ -3,11 +3,36 @@
 // (sign and form as Listing 2); reservoir Eq. (17); compact nine-point TE-TM
 // operator Delta_LT (d_x -+ i d_y)^2 on the other component.
 // Used by the temporally blocked variants (STEP, RESIDENT).  Product code: shares nothing with oracle/.
+//
+// Written on (re, im) PAIRS: for complex fp32 every pair operation below is one packed sm_100 instruction
+// (FADD2 / FMUL2 / FFMA2 on a 64-bit register pair), and multiplication by +-i is an operand modifier of that
+// instruction (swap + one-sided negation), not an instruction.  The pair ops have the same flop throughput as the
+// scalar ones but take half the issue slots, which is what bounds variant STEP (DESIGN.md sections 5.2 and 6).
+// For complex fp64 the same code expands to scalar DADD/DMUL/DFMA.
 #pragma once
 
 #include "phx_common.cuh"
 
 namespace phx {
+
+// ---- pair arithmetic -------------------------------------------------------------------------------------------
+__device__ __forceinline__ float2 add2(float2 a, float2 b) { return __fadd2_rn(a, b); }
+__device__ __forceinline__ float2 sub2(float2 a, float2 b) { return __fadd2_rn(a, make_float2(-b.x, -b.y)); }
+__device__ __forceinline__ float2 fma2(float2 a, float2 b, float2 c) { return __ffma2_rn(a, b, c); }
+__device__ __forceinline__ float2 mul2s(float s, float2 a) { return __fmul2_rn(make_float2(s, s), a); }
+__device__ __forceinline__ float2 fma2s(float s, float2 a, float2 c) { return __ffma2_rn(make_float2(s, s), a, c); }   // s*a + c
+
+__device__ __forceinline__ double2 add2(double2 a, double2 b) { return make_double2(a.x + b.x, a.y + b.y); }
+__device__ __forceinline__ double2 sub2(double2 a, double2 b) { return make_double2(a.x - b.x, a.y - b.y); }
+__device__ __forceinline__ double2 fma2(double2 a, double2 b, double2 c) { return make_double2(fma(a.x, b.x, c.x), fma(a.y, b.y, c.y)); }
+__device__ __forceinline__ double2 mul2s(double s, double2 a) { return make_double2(s * a.x, s * a.y); }
+__device__ __forceinline__ double2 fma2s(double s, double2 a, double2 c) { return make_double2(fma(s, a.x, c.x), fma(s, a.y, c.y)); }
+
+// i*a and -i*a (free operand modifiers of the packed instructions)
+__device__ __forceinline__ float2 rot(float2 a) { return make_float2(-a.y, a.x); }
+__device__ __forceinline__ float2 nrot(float2 a) { return make_float2(a.y, -a.x); }
+__device__ __forceinline__ double2 rot(double2 a) { return make_double2(-a.y, a.x); }
+__device__ __forceinline__ double2 nrot(double2 a) { return make_double2(a.y, -a.x); }
 
 // Nine-point neighbourhood of one component around a cell.  Scalar models read only c, w, e, s, n.
 template <typename T>
@@ -15,37 +40,45 @@ struct Nbhd {
     typename Cx<T>::type c, w, e, s, n, sw, se, nw, ne;   // s = row j-1, n = row j+1, w = column i-1, e = column i+1
 };
 
+// Undivided differences of one component at a cell: A = Dxx, B = Dyy (five-point part), D = Dxy4 (corners).
+template <typename T>
+struct Diff {
+    typename Cx<T>::type A, B, D;
+};
+
+template <typename T, bool NINE>
+__device__ __forceinline__ void differences(const Nbhd<T>& nb, Diff<T>& d) {
+    d.A = fma2s(T(-2), nb.c, add2(nb.e, nb.w));
+    d.B = fma2s(T(-2), nb.c, add2(nb.n, nb.s));
+    if (NINE) d.D = add2(sub2(nb.ne, nb.se), sub2(nb.sw, nb.nw));
+}
+
 // K = i L - i W y + (Rr n / 2 - hgc) y - i J[other],  Kn = P - (gamr + Rr rho) n
-//   own:    neighbourhood of this component (five-point part used)
-//   oth:    neighbourhood of the other component (SPINOR only; all nine points used)
-//   upper:  true for the psi_+ equation (operator (d_x - i d_y)^2 acts on psi_-)
+//   y, own:  this component's value and differences;  yo, oth: the other component's (SPINOR only)
+//   upper:   true for the psi_+ equation (operator (d_x - i d_y)^2 acts on psi_-)
 template <typename T, bool SPINOR, bool RES>
-__device__ __forceinline__ void deriv(const Coef<T>& k, const Nbhd<T>& own, const Nbhd<T>& oth, bool upper, T nres, T V, T P,
-                                      T& Kr, T& Ki, T& Kn) {
-    const auto y = own.c;
-    const T rho = y.x * y.x + y.y * y.y - k.doff;
+__device__ __forceinline__ typename Cx<T>::type deriv(const Coef<T>& k, typename Cx<T>::type y, const Diff<T>& own,
+                                                      typename Cx<T>::type yo, const Diff<T>& oth, bool upper, T nres, T V,
+                                                      T P, T& Kn) {
+    using C = typename Cx<T>::type;
+    const T rho = fma(y.y, y.y, fma(y.x, y.x, -k.doff));
     // (hbar/2m) lap, Eq. (8)
-    const T Lr = k.cx * (own.e.x + own.w.x - T(2) * y.x) + k.cy * (own.n.x + own.s.x - T(2) * y.x);
-    const T Li = k.cx * (own.e.y + own.w.y - T(2) * y.y) + k.cy * (own.n.y + own.s.y - T(2) * y.y);
-    T pot = V + k.g * rho;
-    if (RES) pot += k.gr * nres;
-    if (SPINOR) pot += k.gx * (oth.c.x * oth.c.x + oth.c.y * oth.c.y - k.doff);
+    const C L = fma2s(k.cy, own.B, mul2s(k.cx, own.A));
+    T pot = fma(k.g, rho, V);
+    if (RES) pot = fma(k.gr, nres, pot);
+    if (SPINOR) pot = fma(k.gx, fma(yo.y, yo.y, fma(yo.x, yo.x, -k.doff)), pot);
     const T W = k.ih * pot;
-    const T gain = RES ? (T(0.5) * k.Rr * nres - k.hgc) : -k.hgc;
-    Kr = -Li + W * y.y + gain * y.x;
-    Ki = Lr - W * y.x + gain * y.y;
+    const T gain = RES ? fma(T(0.5) * k.Rr, nres, -k.hgc) : -k.hgc;
+    // i L + gain y - i W y
+    C K = fma2s(-W, rot(y), fma2s(gain, y, rot(L)));
     if (SPINOR) {
-        const auto o = oth.c;
-        const T dxx_r = oth.e.x + oth.w.x - T(2) * o.x, dxx_i = oth.e.y + oth.w.y - T(2) * o.y;
-        const T dyy_r = oth.n.x + oth.s.x - T(2) * o.x, dyy_i = oth.n.y + oth.s.y - T(2) * o.y;
-        const T dxy_r = oth.ne.x - oth.se.x - oth.nw.x + oth.sw.x, dxy_i = oth.ne.y - oth.se.y - oth.nw.y + oth.sw.y;
-        const T sgn = upper ? T(-1) : T(1);
-        const T Jr = k.bxx * dxx_r - k.byy * dyy_r - sgn * k.bxy * dxy_i;
-        const T Ji = k.bxx * dxx_i - k.byy * dyy_i + sgn * k.bxy * dxy_r;
-        Kr += Ji;
-        Ki -= Jr;
+        // -i J,  J = bxx Dxx - byy Dyy -+ i bxy Dxy4 of the other component:  -i bxx A + i byy B -+ bxy D
+        K = fma2s(-k.bxx, rot(oth.A), K);
+        K = fma2s(k.byy, rot(oth.B), K);
+        K = fma2s(upper ? -k.bxy : k.bxy, oth.D, K);
     }
     Kn = RES ? P - (k.gamr + k.Rr * rho) * nres : T(0);
+    return K;
 }
 
 }  // namespace phx

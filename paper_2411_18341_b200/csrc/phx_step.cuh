@@ -280,6 +280,15 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
             const bool in2 = !ZBC || (inx && (!zy || (j - 1 >= 0 && j - 1 < ny)));
             const bool in3 = !ZBC || (inx && (!zy || (j - 2 >= 0 && j - 2 < ny)));
             Nbhd<T> nb[NC][VEC];
+            Diff<T> df[NC][VEC];
+            auto O = [](int s) { return SPINOR ? 1 - s : 0; };            // index of the other component
+            auto diffs = [](const Nbhd<T> (&nb)[NC][VEC], Diff<T> (&df)[NC][VEC]) {
+#pragma unroll
+                for (int s = 0; s < NC; ++s) {
+#pragma unroll
+                    for (int i = 0; i < VEC; ++i) differences<T, SPINOR>(nb[s][i], df[s][i]);
+                }
+            };
 
             // ---- stage 1: K1 on row j from psi rows j-1, j, j+1 (Eq. (2)) ---------------------------------------------
 #pragma unroll
@@ -289,16 +298,17 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
                 for (int i = 0; i < VEC; ++i) { w.r[0][i] = psw[s][1][i]; w.r[1][i] = psw[s][2][i]; w.r[2][i] = psw[s][3][i]; }
                 gather<T, VEC, SPINOR>(w, nb[s]);
             }
+            diffs(nb, df);
 #pragma unroll
             for (int s = 0; s < NC; ++s) {
 #pragma unroll
                 for (int i = 0; i < VEC; ++i) {
-                    T Kr, Ki, Kn;
+                    T Kn;
                     const T nres = RES ? nw[s][0][i] : T(0);
-                    deriv<T, SPINOR, RES>(k, nb[s][i], nb[SPINOR ? 1 - s : 0][i], s == 0, nres, Vw[0][i], Pw[0][i], Kr, Ki, Kn);
+                    const C K = deriv<T, SPINOR, RES>(k, nb[s][i].c, df[s][i], nb[O(s)][i].c, df[O(s)][i], s == 0, nres, Vw[0][i], Pw[0][i], Kn);
                     const C p = psw[s][2][i];
-                    y2[s].r[2][i] = in1 ? mk<T>(p.x + k.hdt * Kr, p.y + k.hdt * Ki) : czero;
-                    accN[s][i] = mk<T>(p.x + k.dt6 * Kr, p.y + k.dt6 * Ki);
+                    y2[s].r[2][i] = in1 ? fma2s(k.hdt, K, p) : czero;
+                    accN[s][i] = fma2s(k.dt6, K, p);
                     if (RES) { n2N[s][i] = nres + k.hdt * Kn; naccN[s][i] = nres + k.dt6 * Kn; }
                 }
             }
@@ -306,15 +316,16 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
             // ---- stage 2: K2 on row j-1 from y2 rows j-2, j-1, j (Eq. (3)) --------------------------------------------
 #pragma unroll
             for (int s = 0; s < NC; ++s) gather<T, VEC, SPINOR>(y2[s], nb[s]);
+            diffs(nb, df);
 #pragma unroll
             for (int s = 0; s < NC; ++s) {
 #pragma unroll
                 for (int i = 0; i < VEC; ++i) {
-                    T Kr, Ki, Kn;
-                    deriv<T, SPINOR, RES>(k, nb[s][i], nb[SPINOR ? 1 - s : 0][i], s == 0, RES ? n2[s][i] : T(0), Vw[1][i], Pw[1][i], Kr, Ki, Kn);
+                    T Kn;
+                    const C K = deriv<T, SPINOR, RES>(k, nb[s][i].c, df[s][i], nb[O(s)][i].c, df[O(s)][i], s == 0, RES ? n2[s][i] : T(0), Vw[1][i], Pw[1][i], Kn);
                     const C p = psw[s][1][i];
-                    y3[s].r[2][i] = in2 ? mk<T>(p.x + k.hdt * Kr, p.y + k.hdt * Ki) : czero;
-                    acc[s][0][i] = mk<T>(acc[s][0][i].x + k.dt3 * Kr, acc[s][0][i].y + k.dt3 * Ki);
+                    y3[s].r[2][i] = in2 ? fma2s(k.hdt, K, p) : czero;
+                    acc[s][0][i] = fma2s(k.dt3, K, acc[s][0][i]);
                     if (RES) { n3N[s][i] = nw[s][1][i] + k.hdt * Kn; nacc[s][0][i] += k.dt3 * Kn; }
                 }
             }
@@ -322,15 +333,16 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
             // ---- stage 3: K3 on row j-2 from y3 rows j-3, j-2, j-1 (Eq. (4)) ------------------------------------------
 #pragma unroll
             for (int s = 0; s < NC; ++s) gather<T, VEC, SPINOR>(y3[s], nb[s]);
+            diffs(nb, df);
 #pragma unroll
             for (int s = 0; s < NC; ++s) {
 #pragma unroll
                 for (int i = 0; i < VEC; ++i) {
-                    T Kr, Ki, Kn;
-                    deriv<T, SPINOR, RES>(k, nb[s][i], nb[SPINOR ? 1 - s : 0][i], s == 0, RES ? n3[s][i] : T(0), Vw[2][i], Pw[2][i], Kr, Ki, Kn);
+                    T Kn;
+                    const C K = deriv<T, SPINOR, RES>(k, nb[s][i].c, df[s][i], nb[O(s)][i].c, df[O(s)][i], s == 0, RES ? n3[s][i] : T(0), Vw[2][i], Pw[2][i], Kn);
                     const C p = psw[s][0][i];
-                    y4[s].r[2][i] = in3 ? mk<T>(p.x + k.dt * Kr, p.y + k.dt * Ki) : czero;
-                    acc[s][1][i] = mk<T>(acc[s][1][i].x + k.dt3 * Kr, acc[s][1][i].y + k.dt3 * Ki);
+                    y4[s].r[2][i] = in3 ? fma2s(k.dt, K, p) : czero;
+                    acc[s][1][i] = fma2s(k.dt3, K, acc[s][1][i]);
                     if (RES) { n4N[s][i] = nw[s][2][i] + k.dt * Kn; nacc[s][1][i] += k.dt3 * Kn; }
                 }
             }
@@ -338,6 +350,7 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
             // ---- stage 4: K4 on row j-3 from y4 rows j-4, j-3, j-2; psi(t+dt) of Eq. (6) (+ dW of Eq. (22)) ----------
 #pragma unroll
             for (int s = 0; s < NC; ++s) gather<T, VEC, SPINOR>(y4[s], nb[s]);
+            diffs(nb, df);
             const int jr = j - 3;
             const bool st_row = jr >= r0 && jr < r1;
 #pragma unroll
@@ -346,9 +359,9 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
                 T nout[VEC];
 #pragma unroll
                 for (int i = 0; i < VEC; ++i) {
-                    T Kr, Ki, Kn;
-                    deriv<T, SPINOR, RES>(k, nb[s][i], nb[SPINOR ? 1 - s : 0][i], s == 0, RES ? n4[s][i] : T(0), Vw[3][i], Pw[3][i], Kr, Ki, Kn);
-                    out[i] = mk<T>(acc[s][2][i].x + k.dt6 * Kr, acc[s][2][i].y + k.dt6 * Ki);
+                    T Kn;
+                    const C K = deriv<T, SPINOR, RES>(k, nb[s][i].c, df[s][i], nb[O(s)][i].c, df[O(s)][i], s == 0, RES ? n4[s][i] : T(0), Vw[3][i], Pw[3][i], Kn);
+                    out[i] = fma2s(k.dt6, K, acc[s][2][i]);
                     nout[i] = RES ? nacc[s][2][i] + k.dt6 * Kn : T(0);
                 }
                 if (st_row && st_lane) {
@@ -360,8 +373,7 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
                             const C xi = s == 0 ? normal_pair(wd.x, wd.y, T(0)) : normal_pair(wd.z, wd.w, T(0));
                             const T nt = RES ? nw[s][3][i] : T(0);      // reservoir at the start of the step
                             const T sigma = sqrt(k.sig2 * (T(2) * k.hgc + k.Rr * nt));
-                            out[i].x += sigma * xi.x;
-                            out[i].y += sigma * xi.y;
+                            out[i] = fma2s(sigma, xi, out[i]);
                         }
                     }
                     const size_t o = boff + (size_t)jr * nx + xl;

@@ -255,8 +255,9 @@ int step_occupancy(const phx_grid* g, int vec) {
     }
 }
 
-// Rows per chunk: every CTA costs (ly + 9) row iterations (4 + 4 halo rows and the pipeline fill), and the grid
-// runs in ceil(CTAs / resident CTAs) waves; pick the chunk count that minimises waves * (ly + 9).
+// Rows per chunk: every CTA costs (ly + 9) row iterations (4 + 4 halo rows and the pipeline fill) rounded up to the
+// unroll factor of the row loop (5, the ring length), and the grid runs in ceil(CTAs / resident CTAs) waves; pick the
+// chunk count that minimises waves * iterations.
 int step_rows_per_chunk(const phx_grid* g, int vec) {
     if (g->step_ly) return g->step_ly < g->d.ny ? g->step_ly : g->d.ny;
     const int strips = (g->d.nx + 32 * vec - 9) / (32 * vec - 8);
@@ -269,7 +270,7 @@ int step_rows_per_chunk(const phx_grid* g, int vec) {
         const int ly = (g->d.ny + nch - 1) / nch;
         const int real_chunks = (g->d.ny + ly - 1) / ly;
         const long waves = (ctas_row * real_chunks + slots - 1) / slots;
-        const long cost = waves * (ly + 9);
+        const long cost = waves * ((ly + 9 + 4) / 5 * 5);
         if (best_cost < 0 || cost < best_cost) { best_cost = cost; best_ly = ly; }
     }
     return best_ly;
@@ -351,7 +352,8 @@ cudaError_t capture(phx_grid* g, int steps, int parity, cudaGraphExec_t* out) {
     return e;
 }
 
-bool step_variant_ok(const phx_grid* g) { return !g->hasE; }   // the fused step carries no drive term
+// The fused step carries no drive term, and addresses a plane by 32-bit cell offsets.
+bool step_variant_ok(const phx_grid* g) { return !g->hasE && (size_t)g->d.nx * (size_t)g->d.ny < ((size_t)1 << 31); }
 
 // AUTO takes the fused step wherever it can run: it is 1.4-3.5x faster than the per-stage kernels on every
 // BASELINE workload; STAGE runs every model, size and term.

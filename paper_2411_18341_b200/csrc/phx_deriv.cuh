@@ -28,11 +28,9 @@ __device__ __forceinline__ double2 fma2(double2 a, double2 b, double2 c) { retur
 __device__ __forceinline__ double2 mul2s(double s, double2 a) { return make_double2(s * a.x, s * a.y); }
 __device__ __forceinline__ double2 fma2s(double s, double2 a, double2 c) { return make_double2(fma(s, a.x, c.x), fma(s, a.y, c.y)); }
 
-// i*a and -i*a (free operand modifiers of the packed instructions)
+// i*a (a free operand modifier of the packed instructions when it is the addend)
 __device__ __forceinline__ float2 rot(float2 a) { return make_float2(-a.y, a.x); }
-__device__ __forceinline__ float2 nrot(float2 a) { return make_float2(a.y, -a.x); }
 __device__ __forceinline__ double2 rot(double2 a) { return make_double2(-a.y, a.x); }
-__device__ __forceinline__ double2 nrot(double2 a) { return make_double2(a.y, -a.x); }
 
 // Nine-point neighbourhood of one component around a cell.  Scalar models read only c, w, e, s, n.
 template <typename T>
@@ -69,14 +67,16 @@ __device__ __forceinline__ typename Cx<T>::type deriv(const Coef<T>& k, typename
     if (SPINOR) pot = fma(k.gx, fma(yo.y, yo.y, fma(yo.x, yo.x, -k.doff)), pot);
     const T W = k.ih * pot;
     const T gain = RES ? fma(T(0.5) * k.Rr, nres, -k.hgc) : -k.hgc;
-    // i L + gain y - i W y
-    C K = fma2s(-W, rot(y), fma2s(gain, y, rot(L)));
+    // K = i M + gain y -+ bxy Dxy4[other],  M = L - W y - bxx Dxx[other] + byy Dyy[other]
+    // (-i J with J = bxx Dxx - byy Dyy -+ i bxy Dxy4 of the other component; the one rotation sits on the addend
+    // operand, where the packed instruction takes it as a modifier)
+    C M = fma2s(-W, y, L);
     if (SPINOR) {
-        // -i J,  J = bxx Dxx - byy Dyy -+ i bxy Dxy4 of the other component:  -i bxx A + i byy B -+ bxy D
-        K = fma2s(-k.bxx, rot(oth.A), K);
-        K = fma2s(k.byy, rot(oth.B), K);
-        K = fma2s(upper ? -k.bxy : k.bxy, oth.D, K);
+        M = fma2s(-k.bxx, oth.A, M);
+        M = fma2s(k.byy, oth.B, M);
     }
+    C K = fma2s(gain, y, rot(M));
+    if (SPINOR) K = fma2s(upper ? -k.bxy : k.bxy, oth.D, K);
     Kn = RES ? P - (k.gamr + k.Rr * rho) * nres : T(0);
     return K;
 }

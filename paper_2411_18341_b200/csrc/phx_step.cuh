@@ -92,42 +92,44 @@ __device__ __forceinline__ float2 dn1(float2 v) { return make_float2(__shfl_down
 __device__ __forceinline__ double2 up1(double2 v) { return make_double2(__shfl_up_sync(0xffffffffu, v.x, 1), __shfl_up_sync(0xffffffffu, v.y, 1)); }
 __device__ __forceinline__ double2 dn1(double2 v) { return make_double2(__shfl_down_sync(0xffffffffu, v.x, 1), __shfl_down_sync(0xffffffffu, v.y, 1)); }
 
-// Three-row window of one component's stage input: r[0] = row below the centre (j-1), r[1] = centre, r[2] = j+1.
-template <typename T, int VEC>
-struct Win3 {
-    typename Cx<T>::type r[3][VEC];
-};
-
-// Neighbourhood of cell i of the centre row of a window; west/east of the lane's cells by shuffle.
-// NINE = false leaves the corners unset (scalar models never read them).
+// Neighbourhood of cell i of the centre row (rc) of a three-row window (rs = row below, rn = row above);
+// west/east of the lane's cells by shuffle.  NINE = false leaves the corners unset (scalar models never read them).
 template <typename T, int VEC, bool NINE>
-__device__ __forceinline__ void gather(const Win3<T, VEC>& w, Nbhd<T> (&nb)[VEC]) {
+__device__ __forceinline__ void gather(const typename Cx<T>::type (&rs)[VEC], const typename Cx<T>::type (&rc)[VEC],
+                                       const typename Cx<T>::type (&rn)[VEC], Nbhd<T> (&nb)[VEC]) {
     using C = typename Cx<T>::type;
     C west[3], east[3];
-#pragma unroll
-    for (int r = 0; r < 3; ++r) {
-        if (NINE || r == 1) {
-            west[r] = up1(w.r[r][VEC - 1]);
-            east[r] = dn1(w.r[r][0]);
-        }
+    west[1] = up1(rc[VEC - 1]);
+    east[1] = dn1(rc[0]);
+    if (NINE) {
+        west[0] = up1(rs[VEC - 1]);
+        east[0] = dn1(rs[0]);
+        west[2] = up1(rn[VEC - 1]);
+        east[2] = dn1(rn[0]);
     }
 #pragma unroll
     for (int i = 0; i < VEC; ++i) {
-        nb[i].c = w.r[1][i];
-        nb[i].s = w.r[0][i];
-        nb[i].n = w.r[2][i];
-        nb[i].w = i == 0 ? west[1] : w.r[1][i - 1];
-        nb[i].e = i == VEC - 1 ? east[1] : w.r[1][i + 1];
+        nb[i].c = rc[i];
+        nb[i].s = rs[i];
+        nb[i].n = rn[i];
+        nb[i].w = i == 0 ? west[1] : rc[i - 1];
+        nb[i].e = i == VEC - 1 ? east[1] : rc[i + 1];
         if (NINE) {
-            nb[i].sw = i == 0 ? west[0] : w.r[0][i - 1];
-            nb[i].se = i == VEC - 1 ? east[0] : w.r[0][i + 1];
-            nb[i].nw = i == 0 ? west[2] : w.r[2][i - 1];
-            nb[i].ne = i == VEC - 1 ? east[2] : w.r[2][i + 1];
+            nb[i].sw = i == 0 ? west[0] : rs[i - 1];
+            nb[i].se = i == VEC - 1 ? east[0] : rs[i + 1];
+            nb[i].nw = i == 0 ? west[2] : rn[i - 1];
+            nb[i].ne = i == VEC - 1 ? east[2] : rn[i + 1];
         }
     }
 }
 
 }  // namespace stepk
+
+// Rows carried in registers live in RINGS of PHX_STEP_RING slots: the row with number q sits in slot q mod RING of
+// its ring for as long as it is live, and the row loop is unrolled RING times, so that every slot index is a
+// compile-time constant and moving the windows down by one row costs no instruction (a dead slot costs no
+// register either).  RING = 5 is the longest life: psi rows j-2 .. j+2 and V rows j-3 .. j+1.
+#define PHX_STEP_RING 5
 
 template <typename T, int VEC, int MODEL, bool NOISE, bool ZBC, int MINB>
 __global__ void __launch_bounds__(128, MINB)
@@ -138,6 +140,7 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
     constexpr bool RES = model_reservoir(MODEL);
     constexpr int NC = SPINOR ? 2 : 1;
     constexpr int W = 32 * VEC, OUTW = W - 8;
+    constexpr int RING = PHX_STEP_RING;
     const Geom& g = a.geo;
     const Coef<T>& k = a.k;
     const int nx = g.nx, ny = g.ny;
@@ -164,252 +167,246 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
     const size_t boff = (size_t)blockIdx.z * g.plane;
     const bool zy = ZBC && g.bc_y;
 
-    // ---- register windows (state carried from one iteration to the next; row numbers relative to the front j) ----
-    const C czero = mk<T>(T(0), T(0));
-    C psw[NC][4][VEC];                      // psi rows j-2, j-1, j, j+1
-    C psn[NC][VEC];                         // psi row j+2, in flight
-    Win3<T, VEC> y2[NC], y3[NC], y4[NC];    // r[0], r[1]: rows (j-2, j-1), (j-3, j-2), (j-4, j-3); r[2] is produced in the iteration
-    C acc[NC][3][VEC];                      // running sum of Eq. (6), rows j-1, j-2, j-3
-    T Vw[4][VEC], Pw[4][VEC];               // V, P rows j, j-1, j-2, j-3
-    T Vn[VEC], Pn[VEC];                     // row j+1, in flight
-    T nw[NC][4][VEC], nn[NC][VEC];          // reservoir state rows j, j-1, j-2, j-3; row j+1 in flight
-    T n2[NC][VEC], n3[NC][VEC], n4[NC][VEC];   // reservoir stage inputs of rows j-1, j-2, j-3 (cell-local)
-    T nacc[NC][3][VEC];                     // reservoir running sum, rows j-1, j-2, j-3
+    // ---- base pointers of this realisation (warp-uniform); rows and columns are addressed by 32-bit cell offsets ----
+    const C* pin[NC];
+    C* pout[NC];
+    const T* nin[NC];
+    T* nout_p[NC];
 #pragma unroll
     for (int s = 0; s < NC; ++s) {
+        pin[s] = a.psi_in[s] + boff;
+        pout[s] = a.psi_out[s] + boff;
+        nin[s] = RES ? a.n_in[s] + boff : nullptr;
+        nout_p[s] = RES ? a.n_out[s] + boff : nullptr;
+    }
+    const T* Vp = a.V;
+    const T* Pp = RES ? a.P : nullptr;
+    // keep the bases as they are: one 64-bit register pair each, every access = base + (32-bit cell offset) * size
+#pragma unroll
+    for (int s = 0; s < NC; ++s) {
+        asm volatile("" : "+l"(pin[s]), "+l"(pout[s]));
+        if (RES) asm volatile("" : "+l"(nin[s]), "+l"(nout_p[s]));
+    }
+    asm volatile("" : "+l"(Vp), "+l"(Pp));
+
+    // ---- register rings (slot of row q = q mod RING; see the note above) ---------------------------------------------
+    const C czero = mk<T>(T(0), T(0));
+    C psr[NC][RING][VEC];                   // psi(t): rows j-2 .. j+1 live, row j+2 in flight
+    C y2r[NC][RING][VEC];                   // stage-2 input: rows j-2, j-1 carried, row j produced
+    C y3r[NC][RING][VEC];                   // stage-3 input: rows j-3, j-2 carried, row j-1 produced
+    C y4r[NC][RING][VEC];                   // stage-4 input: rows j-4, j-3 carried, row j-2 produced
+    C accr[NC][RING][VEC];                  // running sum of Eq. (6): row j produced, rows j-1 .. j-3 updated / consumed
+    T Vr[RING][VEC], Pr[RING][VEC];         // V, P: rows j-3 .. j live, row j+1 in flight
+    T nr[NC][RING][VEC];                    // reservoir n(t): rows j-3 .. j live, row j+1 in flight
+    T n2r[NC][RING][VEC], n3r[NC][RING][VEC], n4r[NC][RING][VEC];   // reservoir stage inputs (cell-local)
+    T naccr[NC][RING][VEC];                 // reservoir running sum
+#pragma unroll
+    for (int r = 0; r < RING; ++r) {
 #pragma unroll
         for (int i = 0; i < VEC; ++i) {
 #pragma unroll
-            for (int r = 0; r < 4; ++r) { psw[s][r][i] = czero; nw[s][r][i] = T(0); }
-#pragma unroll
-            for (int r = 0; r < 3; ++r) { y2[s].r[r][i] = czero; y3[s].r[r][i] = czero; y4[s].r[r][i] = czero; acc[s][r][i] = czero; nacc[s][r][i] = T(0); }
-            psn[s][i] = czero; nn[s][i] = T(0); n2[s][i] = T(0); n3[s][i] = T(0); n4[s][i] = T(0);
+            for (int s = 0; s < NC; ++s) {
+                psr[s][r][i] = czero; y2r[s][r][i] = czero; y3r[s][r][i] = czero; y4r[s][r][i] = czero; accr[s][r][i] = czero;
+                nr[s][r][i] = T(0); n2r[s][r][i] = T(0); n3r[s][r][i] = T(0); n4r[s][r][i] = T(0); naccr[s][r][i] = T(0);
+            }
+            Vr[r][i] = T(0); Pr[r][i] = T(0);
         }
     }
-#pragma unroll
-    for (int i = 0; i < VEC; ++i) {
-#pragma unroll
-        for (int r = 0; r < 4; ++r) { Vw[r][i] = T(0); Pw[r][i] = T(0); }
-        Vn[i] = T(0); Pn[i] = T(0);
-    }
 
-    // wrapped index of the psi row fetched in the first iteration (row r0-4); advanced by one per iteration
-    int qw = r0 - 4;
+    // ---- row bookkeeping: the wrapped index of the row being fetched and the cell offsets (within one plane, < 2^31:
+    // checked by the launch plan) of the lane's first cell in the rows fetched and stored, advanced by one row per iteration
+    const uint32_t plane = (uint32_t)g.plane;
+    int qw = r0 - 4;                        // psi row fetched in the first iteration (row j+2 for j = r0-6)
     if (!zy) { qw %= ny; if (qw < 0) qw += ny; }
-    int qprev = 0;          // wrapped index of the row fetched in the previous iteration (= row j+1 now)
-    bool okprev = false;
-    // rows further ahead are pulled from DRAM into L2 by prefetch instructions (PF_ROWS ahead of the register fetch)
-    constexpr int PF_ROWS = PHX_STEP_PF_ROWS;
-    constexpr int UNROLL_J = PHX_STEP_UNROLL;
-    int qpf = r0 - 4 + PF_ROWS;
-    if (!zy) { qpf %= ny; if (qpf < 0) qpf += ny; }
-    if (PF_ROWS > 0 && inx) {
-        // warm-up: the first PF_ROWS rows of the chunk
-        int q = r0 - 4;
-        if (!zy) { q %= ny; if (q < 0) q += ny; }
-        for (int r = 0; r < PF_ROWS; ++r) {
+    uint32_t ew = (uint32_t)(qw * nx + xg); // cell offset in row qw (modulo 2^32 while the row is outside a zero boundary)
+    uint32_t ewp = 0;                       // cell offset in the row fetched in the previous iteration (row j+1 now)
+    bool okprev = !ZBC;
+    uint32_t est = (uint32_t)((r0 - 9) * nx + xl);   // cell offset in the row stored in this iteration (row j-3), never wrapped
+    // rows further ahead are pulled from DRAM into L2 by prefetch instructions, PF rows ahead of the register fetch
+    // (not across the periodic wrap: those few rows are fetched without a prefetch)
+    constexpr int PF = PHX_STEP_PF_ROWS;
+    const uint32_t epf = (uint32_t)(PF * nx);
+    if (PF > 0 && inx) {
+        // warm-up: the first PF rows of the chunk
+        int q = qw;
+        uint32_t e = ew;
+        for (int r = 0; r < PF; ++r) {
             if (!zy || (q >= 0 && q < ny)) {
-                const size_t o = (size_t)q * nx + xg;
 #pragma unroll
                 for (int s = 0; s < NC; ++s) {
-                    prefetch_l2(a.psi_in[s] + boff + o);
-                    if (RES) prefetch_l2(a.n_in[s] + boff + o);
+                    prefetch_l2(pin[s] + e);
+                    if (RES) prefetch_l2(nin[s] + e);
                 }
-                if (a.V) prefetch_l2(a.V + o);
-                if (RES && a.P) prefetch_l2(a.P + o);
+                if (Vp) prefetch_l2(Vp + e);
+                if (Pp) prefetch_l2(Pp + e);
             }
-            ++q;
-            if (!zy && q == ny) q = 0;
+            ++q; e += nx;
+            if (!zy && q == ny) { q = 0; e -= plane; }
         }
     }
 
-#pragma unroll UNROLL_J
-    for (int j = r0 - 6; j <= r1 + 2; ++j) {
-        if (PF_ROWS > 0) {
-            if (inx && (j + 2 + PF_ROWS <= r1 + 3) && (!zy || (qpf >= 0 && qpf < ny))) {
-                const size_t o = (size_t)qpf * nx + xg;
+#define SL(d) ((ph + (d) + 2 * RING) % RING)     // ring slot of row j+d
+#pragma unroll 1
+    for (int jb = r0 - 6; jb <= r1 + 2; jb += RING) {
 #pragma unroll
-                for (int s = 0; s < NC; ++s) {
-                    prefetch_l2(a.psi_in[s] + boff + o);
-                    if (RES) prefetch_l2(a.n_in[s] + boff + o);
+        for (int ph = 0; ph < RING; ++ph) {
+            const int j = jb + ph;          // front row of this iteration (rows past r1+2 in the last pass: nothing loaded or stored)
+            if (PF > 0) {
+                if (inx && (j + 2 + PF <= r1 + 3) && qw + PF < ny && (!zy || qw + PF >= 0)) {
+#pragma unroll
+                    for (int s = 0; s < NC; ++s) {
+                        prefetch_l2(pin[s] + ew + epf);
+                        if (RES) prefetch_l2(nin[s] + ew + epf);
+                    }
+                    if (Vp) prefetch_l2(Vp + ew + epf);
+                    if (Pp) prefetch_l2(Pp + ew + epf);
                 }
-                if (a.V) prefetch_l2(a.V + o);
-                if (RES && a.P) prefetch_l2(a.P + o);
             }
-            ++qpf;
-            if (!zy && qpf == ny) qpf = 0;
-        }
-        // ---- fetch: psi row j+2; row-local inputs (V, P, n) of row j+1 -----------------------------------------------
-        const bool okq = inx && (j + 2 <= r1 + 3) && (!zy || (qw >= 0 && qw < ny));
-        {
-            const size_t o = (size_t)qw * nx + xg;
+            // ---- fetch: psi row j+2; row-local inputs (V, P, n) of row j+1 -------------------------------------------------
+            // Periodic: every (wrapped) row is readable, so the fetch is unconditional (rows past r1+3 are fetched and not
+            // used).  Zero boundaries: a row or column outside the grid reads as 0.
+            const bool okq = !ZBC || (inx && (j + 2 <= r1 + 3) && (!zy || (qw >= 0 && qw < ny)));
 #pragma unroll
             for (int s = 0; s < NC; ++s) {
+                if (ZBC) {
 #pragma unroll
-                for (int i = 0; i < VEC; ++i) psn[s][i] = czero;
-                if (okq) ldc<VEC>(a.psi_in[s] + boff + o, psn[s]);
+                    for (int i = 0; i < VEC; ++i) psr[s][SL(2)][i] = czero;
+                }
+                if (okq) ldc<VEC>(pin[s] + ew, psr[s][SL(2)]);
             }
-            const size_t op = (size_t)qprev * nx + xg;
+            if (ZBC) {              // (periodic without V or P: the slots keep the zeros they were initialised with)
 #pragma unroll
-            for (int i = 0; i < VEC; ++i) { Vn[i] = T(0); Pn[i] = T(0); }
+                for (int i = 0; i < VEC; ++i) { Vr[SL(1)][i] = T(0); Pr[SL(1)][i] = T(0); }
+            }
             if (okprev) {
-                if (a.V) ldr<VEC>(a.V + op, Vn);
-                if (RES && a.P) ldr<VEC>(a.P + op, Pn);
+                if (Vp) ldr<VEC>(Vp + ewp, Vr[SL(1)]);
+                if (Pp) ldr<VEC>(Pp + ewp, Pr[SL(1)]);
             }
             if constexpr (RES) {
 #pragma unroll
                 for (int s = 0; s < NC; ++s) {
+                    if (ZBC) {
 #pragma unroll
-                    for (int i = 0; i < VEC; ++i) nn[s][i] = T(0);
-                    if (okprev) ldr<VEC>(a.n_in[s] + boff + op, nn[s]);
+                        for (int i = 0; i < VEC; ++i) nr[s][SL(1)][i] = T(0);
+                    }
+                    if (okprev) ldr<VEC>(nin[s] + ewp, nr[s][SL(1)]);
                 }
             }
-        }
 
-        C accN[NC][VEC];
-        T n2N[NC][VEC], n3N[NC][VEC], n4N[NC][VEC], naccN[NC][VEC];
+            if (j >= r0 - 3) {
+                // in-domain flags of the rows whose next stage input is written (zero boundaries: 0 outside the grid)
+                const bool in1 = !ZBC || (inx && (!zy || (j >= 0 && j < ny)));
+                const bool in2 = !ZBC || (inx && (!zy || (j - 1 >= 0 && j - 1 < ny)));
+                const bool in3 = !ZBC || (inx && (!zy || (j - 2 >= 0 && j - 2 < ny)));
+                Nbhd<T> nb[NC][VEC];
+                Diff<T> df[NC][VEC];
+                auto O = [](int s) { return SPINOR ? 1 - s : 0; };            // index of the other component
+                auto diffs = [](const Nbhd<T> (&nb)[NC][VEC], Diff<T> (&df)[NC][VEC]) {
 #pragma unroll
-        for (int s = 0; s < NC; ++s) {
+                    for (int s = 0; s < NC; ++s) {
 #pragma unroll
-            for (int i = 0; i < VEC; ++i) { accN[s][i] = czero; n2N[s][i] = T(0); n3N[s][i] = T(0); n4N[s][i] = T(0); naccN[s][i] = T(0); }
-        }
+                        for (int i = 0; i < VEC; ++i) differences<T, SPINOR>(nb[s][i], df[s][i]);
+                    }
+                };
 
-        if (j >= r0 - 3) {
-            // in-domain flags of the rows whose next stage input is written (zero boundaries: 0 outside the grid)
-            const bool in1 = !ZBC || (inx && (!zy || (j >= 0 && j < ny)));
-            const bool in2 = !ZBC || (inx && (!zy || (j - 1 >= 0 && j - 1 < ny)));
-            const bool in3 = !ZBC || (inx && (!zy || (j - 2 >= 0 && j - 2 < ny)));
-            Nbhd<T> nb[NC][VEC];
-            Diff<T> df[NC][VEC];
-            auto O = [](int s) { return SPINOR ? 1 - s : 0; };            // index of the other component
-            auto diffs = [](const Nbhd<T> (&nb)[NC][VEC], Diff<T> (&df)[NC][VEC]) {
+                // ---- stage 1: K1 on row j from psi rows j-1, j, j+1 (Eq. (2)) ---------------------------------------------
+#pragma unroll
+                for (int s = 0; s < NC; ++s) gather<T, VEC, SPINOR>(psr[s][SL(-1)], psr[s][SL(0)], psr[s][SL(1)], nb[s]);
+                diffs(nb, df);
 #pragma unroll
                 for (int s = 0; s < NC; ++s) {
 #pragma unroll
-                    for (int i = 0; i < VEC; ++i) differences<T, SPINOR>(nb[s][i], df[s][i]);
-                }
-            };
-
-            // ---- stage 1: K1 on row j from psi rows j-1, j, j+1 (Eq. (2)) ---------------------------------------------
-#pragma unroll
-            for (int s = 0; s < NC; ++s) {
-                Win3<T, VEC> w;
-#pragma unroll
-                for (int i = 0; i < VEC; ++i) { w.r[0][i] = psw[s][1][i]; w.r[1][i] = psw[s][2][i]; w.r[2][i] = psw[s][3][i]; }
-                gather<T, VEC, SPINOR>(w, nb[s]);
-            }
-            diffs(nb, df);
-#pragma unroll
-            for (int s = 0; s < NC; ++s) {
-#pragma unroll
-                for (int i = 0; i < VEC; ++i) {
-                    T Kn;
-                    const T nres = RES ? nw[s][0][i] : T(0);
-                    const C K = deriv<T, SPINOR, RES>(k, nb[s][i].c, df[s][i], nb[O(s)][i].c, df[O(s)][i], s == 0, nres, Vw[0][i], Pw[0][i], Kn);
-                    const C p = psw[s][2][i];
-                    y2[s].r[2][i] = in1 ? fma2s(k.hdt, K, p) : czero;
-                    accN[s][i] = fma2s(k.dt6, K, p);
-                    if (RES) { n2N[s][i] = nres + k.hdt * Kn; naccN[s][i] = nres + k.dt6 * Kn; }
-                }
-            }
-
-            // ---- stage 2: K2 on row j-1 from y2 rows j-2, j-1, j (Eq. (3)) --------------------------------------------
-#pragma unroll
-            for (int s = 0; s < NC; ++s) gather<T, VEC, SPINOR>(y2[s], nb[s]);
-            diffs(nb, df);
-#pragma unroll
-            for (int s = 0; s < NC; ++s) {
-#pragma unroll
-                for (int i = 0; i < VEC; ++i) {
-                    T Kn;
-                    const C K = deriv<T, SPINOR, RES>(k, nb[s][i].c, df[s][i], nb[O(s)][i].c, df[O(s)][i], s == 0, RES ? n2[s][i] : T(0), Vw[1][i], Pw[1][i], Kn);
-                    const C p = psw[s][1][i];
-                    y3[s].r[2][i] = in2 ? fma2s(k.hdt, K, p) : czero;
-                    acc[s][0][i] = fma2s(k.dt3, K, acc[s][0][i]);
-                    if (RES) { n3N[s][i] = nw[s][1][i] + k.hdt * Kn; nacc[s][0][i] += k.dt3 * Kn; }
-                }
-            }
-
-            // ---- stage 3: K3 on row j-2 from y3 rows j-3, j-2, j-1 (Eq. (4)) ------------------------------------------
-#pragma unroll
-            for (int s = 0; s < NC; ++s) gather<T, VEC, SPINOR>(y3[s], nb[s]);
-            diffs(nb, df);
-#pragma unroll
-            for (int s = 0; s < NC; ++s) {
-#pragma unroll
-                for (int i = 0; i < VEC; ++i) {
-                    T Kn;
-                    const C K = deriv<T, SPINOR, RES>(k, nb[s][i].c, df[s][i], nb[O(s)][i].c, df[O(s)][i], s == 0, RES ? n3[s][i] : T(0), Vw[2][i], Pw[2][i], Kn);
-                    const C p = psw[s][0][i];
-                    y4[s].r[2][i] = in3 ? fma2s(k.dt, K, p) : czero;
-                    acc[s][1][i] = fma2s(k.dt3, K, acc[s][1][i]);
-                    if (RES) { n4N[s][i] = nw[s][2][i] + k.dt * Kn; nacc[s][1][i] += k.dt3 * Kn; }
-                }
-            }
-
-            // ---- stage 4: K4 on row j-3 from y4 rows j-4, j-3, j-2; psi(t+dt) of Eq. (6) (+ dW of Eq. (22)) ----------
-#pragma unroll
-            for (int s = 0; s < NC; ++s) gather<T, VEC, SPINOR>(y4[s], nb[s]);
-            diffs(nb, df);
-            const int jr = j - 3;
-            const bool st_row = jr >= r0 && jr < r1;
-#pragma unroll
-            for (int s = 0; s < NC; ++s) {
-                C out[VEC];
-                T nout[VEC];
-#pragma unroll
-                for (int i = 0; i < VEC; ++i) {
-                    T Kn;
-                    const C K = deriv<T, SPINOR, RES>(k, nb[s][i].c, df[s][i], nb[O(s)][i].c, df[O(s)][i], s == 0, RES ? n4[s][i] : T(0), Vw[3][i], Pw[3][i], Kn);
-                    out[i] = fma2s(k.dt6, K, acc[s][2][i]);
-                    nout[i] = RES ? nacc[s][2][i] + k.dt6 * Kn : T(0);
-                }
-                if (st_row && st_lane) {
-                    if (NOISE) {
-#pragma unroll
-                        for (int i = 0; i < VEC; ++i) {
-                            const uint32_t cell = (uint32_t)jr * (uint32_t)nx + (uint32_t)(xl + i);
-                            const uint4 wd = noise_words(a.seed, blockIdx.z, step, cell);
-                            const C xi = s == 0 ? normal_pair(wd.x, wd.y, T(0)) : normal_pair(wd.z, wd.w, T(0));
-                            const T nt = RES ? nw[s][3][i] : T(0);      // reservoir at the start of the step
-                            const T sigma = sqrt(k.sig2 * (T(2) * k.hgc + k.Rr * nt));
-                            out[i] = fma2s(sigma, xi, out[i]);
-                        }
+                    for (int i = 0; i < VEC; ++i) {
+                        T Kn;
+                        const T nres = RES ? nr[s][SL(0)][i] : T(0);
+                        const C K = deriv<T, SPINOR, RES>(k, nb[s][i].c, df[s][i], nb[O(s)][i].c, df[O(s)][i], s == 0, nres, Vr[SL(0)][i], Pr[SL(0)][i], Kn);
+                        const C p = psr[s][SL(0)][i];
+                        y2r[s][SL(0)][i] = in1 ? fma2s(k.hdt, K, p) : czero;
+                        accr[s][SL(0)][i] = fma2s(k.dt6, K, p);
+                        if (RES) { n2r[s][SL(0)][i] = nres + k.hdt * Kn; naccr[s][SL(0)][i] = nres + k.dt6 * Kn; }
                     }
-                    const size_t o = boff + (size_t)jr * nx + xl;
-                    stc<VEC>(a.psi_out[s] + o, out);
-                    if constexpr (RES) str<VEC>(a.n_out[s] + o, nout);
                 }
-            }
-        }
 
-        // ---- slide every window by one row -----------------------------------------------------------------------------
+                // ---- stage 2: K2 on row j-1 from y2 rows j-2, j-1, j (Eq. (3)) --------------------------------------------
 #pragma unroll
-        for (int s = 0; s < NC; ++s) {
+                for (int s = 0; s < NC; ++s) gather<T, VEC, SPINOR>(y2r[s][SL(-2)], y2r[s][SL(-1)], y2r[s][SL(0)], nb[s]);
+                diffs(nb, df);
 #pragma unroll
-            for (int i = 0; i < VEC; ++i) {
-                psw[s][0][i] = psw[s][1][i]; psw[s][1][i] = psw[s][2][i]; psw[s][2][i] = psw[s][3][i]; psw[s][3][i] = psn[s][i];
-                y2[s].r[0][i] = y2[s].r[1][i]; y2[s].r[1][i] = y2[s].r[2][i];
-                y3[s].r[0][i] = y3[s].r[1][i]; y3[s].r[1][i] = y3[s].r[2][i];
-                y4[s].r[0][i] = y4[s].r[1][i]; y4[s].r[1][i] = y4[s].r[2][i];
-                acc[s][2][i] = acc[s][1][i]; acc[s][1][i] = acc[s][0][i]; acc[s][0][i] = accN[s][i];
-                if (RES) {
-                    nw[s][3][i] = nw[s][2][i]; nw[s][2][i] = nw[s][1][i]; nw[s][1][i] = nw[s][0][i]; nw[s][0][i] = nn[s][i];
-                    n4[s][i] = n4N[s][i]; n3[s][i] = n3N[s][i]; n2[s][i] = n2N[s][i];
-                    nacc[s][2][i] = nacc[s][1][i]; nacc[s][1][i] = nacc[s][0][i]; nacc[s][0][i] = naccN[s][i];
+                for (int s = 0; s < NC; ++s) {
+#pragma unroll
+                    for (int i = 0; i < VEC; ++i) {
+                        T Kn;
+                        const T nres = RES ? n2r[s][SL(-1)][i] : T(0);
+                        const C K = deriv<T, SPINOR, RES>(k, nb[s][i].c, df[s][i], nb[O(s)][i].c, df[O(s)][i], s == 0, nres, Vr[SL(-1)][i], Pr[SL(-1)][i], Kn);
+                        const C p = psr[s][SL(-1)][i];
+                        y3r[s][SL(-1)][i] = in2 ? fma2s(k.hdt, K, p) : czero;
+                        accr[s][SL(-1)][i] = fma2s(k.dt3, K, accr[s][SL(-1)][i]);
+                        if (RES) { n3r[s][SL(-1)][i] = nr[s][SL(-1)][i] + k.hdt * Kn; naccr[s][SL(-1)][i] += k.dt3 * Kn; }
+                    }
+                }
+
+                // ---- stage 3: K3 on row j-2 from y3 rows j-3, j-2, j-1 (Eq. (4)) ------------------------------------------
+#pragma unroll
+                for (int s = 0; s < NC; ++s) gather<T, VEC, SPINOR>(y3r[s][SL(-3)], y3r[s][SL(-2)], y3r[s][SL(-1)], nb[s]);
+                diffs(nb, df);
+#pragma unroll
+                for (int s = 0; s < NC; ++s) {
+#pragma unroll
+                    for (int i = 0; i < VEC; ++i) {
+                        T Kn;
+                        const T nres = RES ? n3r[s][SL(-2)][i] : T(0);
+                        const C K = deriv<T, SPINOR, RES>(k, nb[s][i].c, df[s][i], nb[O(s)][i].c, df[O(s)][i], s == 0, nres, Vr[SL(-2)][i], Pr[SL(-2)][i], Kn);
+                        const C p = psr[s][SL(-2)][i];
+                        y4r[s][SL(-2)][i] = in3 ? fma2s(k.dt, K, p) : czero;
+                        accr[s][SL(-2)][i] = fma2s(k.dt3, K, accr[s][SL(-2)][i]);
+                        if (RES) { n4r[s][SL(-2)][i] = nr[s][SL(-2)][i] + k.dt * Kn; naccr[s][SL(-2)][i] += k.dt3 * Kn; }
+                    }
+                }
+
+                // ---- stage 4: K4 on row j-3 from y4 rows j-4, j-3, j-2; psi(t+dt) of Eq. (6) (+ dW of Eq. (22)) ----------
+#pragma unroll
+                for (int s = 0; s < NC; ++s) gather<T, VEC, SPINOR>(y4r[s][SL(-4)], y4r[s][SL(-3)], y4r[s][SL(-2)], nb[s]);
+                diffs(nb, df);
+                const int jr = j - 3;
+                const bool st_row = jr >= r0 && jr < r1;
+#pragma unroll
+                for (int s = 0; s < NC; ++s) {
+                    C out[VEC];
+                    T nout[VEC];
+#pragma unroll
+                    for (int i = 0; i < VEC; ++i) {
+                        T Kn;
+                        const T nres = RES ? n4r[s][SL(-3)][i] : T(0);
+                        const C K = deriv<T, SPINOR, RES>(k, nb[s][i].c, df[s][i], nb[O(s)][i].c, df[O(s)][i], s == 0, nres, Vr[SL(-3)][i], Pr[SL(-3)][i], Kn);
+                        out[i] = fma2s(k.dt6, K, accr[s][SL(-3)][i]);
+                        nout[i] = RES ? naccr[s][SL(-3)][i] + k.dt6 * Kn : T(0);
+                    }
+                    if (st_row && st_lane) {
+                        if (NOISE) {
+#pragma unroll
+                            for (int i = 0; i < VEC; ++i) {
+                                const uint32_t cell = (uint32_t)jr * (uint32_t)nx + (uint32_t)(xl + i);
+                                const uint4 wd = noise_words(a.seed, blockIdx.z, step, cell);
+                                const C xi = s == 0 ? normal_pair(wd.x, wd.y, T(0)) : normal_pair(wd.z, wd.w, T(0));
+                                const T nt = RES ? nr[s][SL(-3)][i] : T(0);      // reservoir at the start of the step
+                                const T sigma = sqrt(k.sig2 * (T(2) * k.hgc + k.Rr * nt));
+                                out[i] = fma2s(sigma, xi, out[i]);
+                            }
+                        }
+                        stc<VEC>(pout[s] + est, out);
+                        if constexpr (RES) str<VEC>(nout_p[s] + est, nout);
+                    }
                 }
             }
+
+            // ---- next row -----------------------------------------------------------------------------------------------
+            ewp = ew;
+            okprev = okq;
+            ++qw; ew += nx; est += nx;
+            if (!zy && qw == ny) { qw = 0; ew -= plane; }
         }
-#pragma unroll
-        for (int i = 0; i < VEC; ++i) {
-            Vw[3][i] = Vw[2][i]; Vw[2][i] = Vw[1][i]; Vw[1][i] = Vw[0][i]; Vw[0][i] = Vn[i];
-            Pw[3][i] = Pw[2][i]; Pw[2][i] = Pw[1][i]; Pw[1][i] = Pw[0][i]; Pw[0][i] = Pn[i];
-        }
-        qprev = qw;
-        okprev = okq;
-        ++qw;
-        if (!zy && qw == ny) qw = 0;
     }
+#undef SL
 }
 
 }  // namespace phx

@@ -18,7 +18,9 @@ typedef double real_t;
 // Resident CTAs (of 4 warps) per SM the register budget is sized for: the carried register windows grow with the
 // number of components and reservoirs (DESIGN.md section 5.2 has the count per model).
 #if PHX_INST_PREC == 32
+#ifndef PHX_MINB_V2
 #define PHX_MINB_V2 (PHX_INST_MODEL == 0 ? 4 : (PHX_INST_MODEL == 1 ? 3 : 2))
+#endif
 #define PHX_MINB_V1 (PHX_INST_MODEL == 0 ? 6 : (PHX_INST_MODEL == 1 ? 5 : 3))
 #else
 #define PHX_MINB_V2 2

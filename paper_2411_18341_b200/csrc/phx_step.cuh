@@ -216,16 +216,17 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
     // ---- row bookkeeping: the wrapped index of the row being fetched and the cell offsets (within one plane, < 2^31:
     // checked by the launch plan) of the lane's first cell in the rows fetched and stored, advanced by one row per iteration
     const uint32_t plane = (uint32_t)g.plane;
-    int qw = r0 - 4;                        // psi row fetched in the first iteration (row j+2 for j = r0-6)
+    const int j0 = r0 - 3;                  // first front row: stage 1 starts on row r0-3, stage 4 reaches row r0 three rows later
+    int qw = j0 - 1;                        // row being fetched (wrapped unless outside a zero boundary)
     if (!zy) { qw %= ny; if (qw < 0) qw += ny; }
-    uint32_t ew = (uint32_t)(qw * nx + xg); // cell offset in row qw (modulo 2^32 while the row is outside a zero boundary)
-    uint32_t ewp = 0;                       // cell offset in the row fetched in the previous iteration (row j+1 now)
+    uint32_t ew = (uint32_t)(qw * nx + xg); // its cell offset (modulo 2^32 while the row is outside a zero boundary)
+    uint32_t ewp = 0;                       // cell offset of the row fetched before it
     bool okprev = !ZBC;
-    uint32_t est = (uint32_t)((r0 - 9) * nx + xl);   // cell offset in the row stored in this iteration (row j-3), never wrapped
+    uint32_t est = (uint32_t)((j0 - 3) * nx + xl);   // cell offset in the row stored in this iteration (row j-3), never wrapped
     // rows further ahead are pulled from DRAM into L2 by prefetch instructions, PF rows ahead of the register fetch
-    // (not across the periodic wrap: those few rows are fetched without a prefetch)
     constexpr int PF = PHX_STEP_PF_ROWS;
-    const uint32_t epf = (uint32_t)(PF * nx);
+    const int pfr = ny >= PF ? PF : 0;      // (a grid shorter than the prefetch distance prefetches the row it is fetching)
+    const uint32_t epf = (uint32_t)(pfr * nx);
     if (PF > 0 && inx) {
         // warm-up: the first PF rows of the chunk
         int q = qw;
@@ -245,14 +246,49 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
         }
     }
 
+    // ---- pipeline fill: psi rows j0-1, j0, j0+1 and the row-local inputs (V, P, n) of row j0 ----------------------------------
+#pragma unroll
+    for (int d = -1; d <= 1; ++d) {
+        constexpr int R2 = 2 * RING;
+        const bool okq = !ZBC || (inx && (!zy || (qw >= 0 && qw < ny)));
+#pragma unroll
+        for (int s = 0; s < NC; ++s) {
+            if (okq) ldc<VEC>(pin[s] + ew, psr[s][(d + R2) % RING]);
+        }
+        if (d == 0 && okq) {
+            if (Vp) ldr<VEC>(Vp + ew, Vr[(d + R2) % RING]);
+            if (Pp) ldr<VEC>(Pp + ew, Pr[(d + R2) % RING]);
+            if constexpr (RES) {
+#pragma unroll
+                for (int s = 0; s < NC; ++s) ldr<VEC>(nin[s] + ew, nr[s][(d + R2) % RING]);
+            }
+        }
+        ewp = ew;
+        okprev = okq;
+        ++qw; ew += nx;
+        if (!zy && qw == ny) { qw = 0; ew -= plane; }
+    }
+
+    // ---- row loop: one pass = RING front rows j0 + RING*k + ph.  Each phase is straight-line code (no branch around the
+    // fetch or the four stages), so that the scheduler sees the loads and their consumers in one block. -------------------------
 #define SL(d) ((ph + (d) + 2 * RING) % RING)     // ring slot of row j+d
 #pragma unroll 1
-    for (int jb = r0 - 6; jb <= r1 + 2; jb += RING) {
+    for (int jb = j0; jb <= r1 + 2; jb += RING) {
 #pragma unroll
         for (int ph = 0; ph < RING; ++ph) {
-            const int j = jb + ph;          // front row of this iteration (rows past r1+2 in the last pass: nothing loaded or stored)
+            const int j = jb + ph;          // front row of this iteration (rows past r1+2 in the last pass are computed and not stored)
             if (PF > 0) {
-                if (inx && (j + 2 + PF <= r1 + 3) && qw + PF < ny && (!zy || qw + PF >= 0)) {
+                if (!ZBC) {
+                    uint32_t e = ew + epf;                   // row qw + pfr, wrapped
+                    if (qw + pfr >= ny) e -= plane;
+#pragma unroll
+                    for (int s = 0; s < NC; ++s) {
+                        prefetch_l2(pin[s] + e);
+                        if (RES) prefetch_l2(nin[s] + e);
+                    }
+                    if (Vp) prefetch_l2(Vp + e);
+                    if (Pp) prefetch_l2(Pp + e);
+                } else if (inx && (j + 2 + pfr <= r1 + 3) && qw + pfr < ny && qw + pfr >= 0) {
 #pragma unroll
                     for (int s = 0; s < NC; ++s) {
                         prefetch_l2(pin[s] + ew + epf);
@@ -293,7 +329,7 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
                 }
             }
 
-            if (j >= r0 - 3) {
+            {
                 // in-domain flags of the rows whose next stage input is written (zero boundaries: 0 outside the grid)
                 const bool in1 = !ZBC || (inx && (!zy || (j >= 0 && j < ny)));
                 const bool in2 = !ZBC || (inx && (!zy || (j - 1 >= 0 && j - 1 < ny)));

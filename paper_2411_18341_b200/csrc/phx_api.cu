@@ -237,21 +237,24 @@ int step_vec(const phx_grid* g) {
     return (g->d.prec == PHX_C32 && g->d.nx % 2 == 0) ? 2 : 1;
 }
 
+// dx == dy: the isotropic form of the Laplacian (cx == cy bit for bit, both derived from the same expression)
+bool step_iso(const phx_grid* g) { return g->d.dx == g->d.dy; }
+
 int step_occupancy(const phx_grid* g, int vec) {
-    const bool noise = g->d.noise != 0, zbc = g->d.bc_x || g->d.bc_y;
+    const bool noise = g->d.noise != 0, zbc = g->d.bc_x || g->d.bc_y, iso = step_iso(g);
     if (g->d.prec == PHX_C32) {
         switch (g->d.model) {
-            case 0: return occupancy_step_32_0(noise, zbc, vec);
-            case 1: return occupancy_step_32_1(noise, zbc, vec);
-            case 2: return occupancy_step_32_2(noise, zbc, vec);
-            default: return occupancy_step_32_3(noise, zbc, vec);
+            case 0: return occupancy_step_32_0(noise, zbc, iso, vec);
+            case 1: return occupancy_step_32_1(noise, zbc, iso, vec);
+            case 2: return occupancy_step_32_2(noise, zbc, iso, vec);
+            default: return occupancy_step_32_3(noise, zbc, iso, vec);
         }
     }
     switch (g->d.model) {
-        case 0: return occupancy_step_64_0(noise, zbc, vec);
-        case 1: return occupancy_step_64_1(noise, zbc, vec);
-        case 2: return occupancy_step_64_2(noise, zbc, vec);
-        default: return occupancy_step_64_3(noise, zbc, vec);
+        case 0: return occupancy_step_64_0(noise, zbc, iso, vec);
+        case 1: return occupancy_step_64_1(noise, zbc, iso, vec);
+        case 2: return occupancy_step_64_2(noise, zbc, iso, vec);
+        default: return occupancy_step_64_3(noise, zbc, iso, vec);
     }
 }
 
@@ -261,7 +264,7 @@ int step_occupancy(const phx_grid* g, int vec) {
 int step_rows_per_chunk(const phx_grid* g, int vec) {
     if (g->step_ly) return g->step_ly < g->d.ny ? g->step_ly : g->d.ny;
     const int strips = (g->d.nx + 32 * vec - 9) / (32 * vec - 8);
-    const long ctas_row = (long)((strips + 3) / 4) * g->d.batch;
+    const long ctas_row = (long)((strips + PHX_STEP_WARPS - 1) / PHX_STEP_WARPS) * g->d.batch;
     const long slots = (long)g->n_sm * step_occupancy(g, vec);
     long best_cost = -1;
     int best_ly = g->d.ny;
@@ -306,22 +309,22 @@ cudaError_t enqueue_step_fused(phx_grid* g, cudaStream_t st, int parity) {
     const int vec = step_vec(g);
     a.strips = (g->d.nx + 32 * vec - 9) / (32 * vec - 8);
     a.ly = step_rows_per_chunk(g, vec);
-    const dim3 grid((a.strips + 3) / 4, (g->d.ny + a.ly - 1) / a.ly, g->d.batch);
+    const dim3 grid((a.strips + PHX_STEP_WARPS - 1) / PHX_STEP_WARPS, (g->d.ny + a.ly - 1) / a.ly, g->d.batch);
     if (grid.y > 65535u) return cudaErrorInvalidConfiguration;
-    const bool noise = g->d.noise != 0, zbc = g->d.bc_x || g->d.bc_y;
+    const bool noise = g->d.noise != 0, zbc = g->d.bc_x || g->d.bc_y, iso = step_iso(g);
     if constexpr (sizeof(T) == 4) {
         switch (g->d.model) {
-            case 0: return launch_step_32_0(a, noise, zbc, vec, grid, st);
-            case 1: return launch_step_32_1(a, noise, zbc, vec, grid, st);
-            case 2: return launch_step_32_2(a, noise, zbc, vec, grid, st);
-            default: return launch_step_32_3(a, noise, zbc, vec, grid, st);
+            case 0: return launch_step_32_0(a, noise, zbc, iso, vec, grid, st);
+            case 1: return launch_step_32_1(a, noise, zbc, iso, vec, grid, st);
+            case 2: return launch_step_32_2(a, noise, zbc, iso, vec, grid, st);
+            default: return launch_step_32_3(a, noise, zbc, iso, vec, grid, st);
         }
     } else {
         switch (g->d.model) {
-            case 0: return launch_step_64_0(a, noise, zbc, vec, grid, st);
-            case 1: return launch_step_64_1(a, noise, zbc, vec, grid, st);
-            case 2: return launch_step_64_2(a, noise, zbc, vec, grid, st);
-            default: return launch_step_64_3(a, noise, zbc, vec, grid, st);
+            case 0: return launch_step_64_0(a, noise, zbc, iso, vec, grid, st);
+            case 1: return launch_step_64_1(a, noise, zbc, iso, vec, grid, st);
+            case 2: return launch_step_64_2(a, noise, zbc, iso, vec, grid, st);
+            default: return launch_step_64_3(a, noise, zbc, iso, vec, grid, st);
         }
     }
 }

@@ -38,16 +38,24 @@ struct Nbhd {
     typename Cx<T>::type c, w, e, s, n, sw, se, nw, ne;   // s = row j-1, n = row j+1, w = column i-1, e = column i+1
 };
 
-// Undivided differences of one component at a cell: A = Dxx, B = Dyy (five-point part), D = Dxy4 (corners).
+// Differences of one component at a cell: L = (hbar/2m) lap, Eq. (8); for the TE-TM operator also the undivided
+// A = Dxx, B = Dyy and D = Dxy4 (corners).
 template <typename T>
 struct Diff {
-    typename Cx<T>::type A, B, D;
+    typename Cx<T>::type L, A, B, D;
 };
 
-template <typename T, bool NINE>
-__device__ __forceinline__ void differences(const Nbhd<T>& nb, Diff<T>& d) {
-    d.A = fma2s(T(-2), nb.c, add2(nb.e, nb.w));
-    d.B = fma2s(T(-2), nb.c, add2(nb.n, nb.s));
+// NINE: the spinor models (all nine points, A, B, D kept).  ISO: dx == dy, so cx == cy and
+// L = cx ((e + w) + (n + s) - 4 c) -- one packed operation fewer, exact factors only.
+template <typename T, bool NINE, bool ISO>
+__device__ __forceinline__ void differences(const Coef<T>& k, const Nbhd<T>& nb, Diff<T>& d) {
+    if (ISO && !NINE) {
+        d.L = mul2s(k.cx, fma2s(T(-4), nb.c, add2(add2(nb.e, nb.w), add2(nb.n, nb.s))));
+    } else {
+        d.A = fma2s(T(-2), nb.c, add2(nb.e, nb.w));
+        d.B = fma2s(T(-2), nb.c, add2(nb.n, nb.s));
+        d.L = fma2s(k.cy, d.B, mul2s(k.cx, d.A));
+    }
     if (NINE) d.D = add2(sub2(nb.ne, nb.se), sub2(nb.sw, nb.nw));
 }
 
@@ -60,8 +68,6 @@ __device__ __forceinline__ typename Cx<T>::type deriv(const Coef<T>& k, typename
                                                       T P, T& Kn) {
     using C = typename Cx<T>::type;
     const T rho = fma(y.y, y.y, fma(y.x, y.x, -k.doff));
-    // (hbar/2m) lap, Eq. (8)
-    const C L = fma2s(k.cy, own.B, mul2s(k.cx, own.A));
     T pot = fma(k.g, rho, V);
     if (RES) pot = fma(k.gr, nres, pot);
     if (SPINOR) pot = fma(k.gx, fma(yo.y, yo.y, fma(yo.x, yo.x, -k.doff)), pot);
@@ -70,7 +76,7 @@ __device__ __forceinline__ typename Cx<T>::type deriv(const Coef<T>& k, typename
     // K = i M + gain y -+ bxy Dxy4[other],  M = L - W y - bxx Dxx[other] + byy Dyy[other]
     // (-i J with J = bxx Dxx - byy Dyy -+ i bxy Dxy4 of the other component; the one rotation sits on the addend
     // operand, where the packed instruction takes it as a modifier)
-    C M = fma2s(-W, y, L);
+    C M = fma2s(-W, y, own.L);
     if (SPINOR) {
         M = fma2s(-k.bxx, oth.A, M);
         M = fma2s(k.byy, oth.B, M);

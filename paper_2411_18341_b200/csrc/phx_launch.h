@@ -3,6 +3,11 @@
 
 #include "phx_common.cuh"
 
+// Warps per CTA of variant STEP (the warps of a CTA are independent: adjacent strips, no shared memory, no barrier).
+#ifndef PHX_STEP_WARPS
+#define PHX_STEP_WARPS 2
+#endif
+
 namespace phx {
 
 template <typename T> struct StageArgs;
@@ -19,14 +24,14 @@ PHX_DECL_STAGE(64, double)
 template <typename T> struct StepArgs;
 
 #define PHX_DECL_STEP(P, T)                                                                                      \
-    cudaError_t launch_step_##P##_0(const StepArgs<T>&, bool noise, bool zbc, int vec, dim3 grid, cudaStream_t); \
-    cudaError_t launch_step_##P##_1(const StepArgs<T>&, bool noise, bool zbc, int vec, dim3 grid, cudaStream_t); \
-    cudaError_t launch_step_##P##_2(const StepArgs<T>&, bool noise, bool zbc, int vec, dim3 grid, cudaStream_t); \
-    cudaError_t launch_step_##P##_3(const StepArgs<T>&, bool noise, bool zbc, int vec, dim3 grid, cudaStream_t); \
-    int occupancy_step_##P##_0(bool noise, bool zbc, int vec);                                                    \
-    int occupancy_step_##P##_1(bool noise, bool zbc, int vec);                                                    \
-    int occupancy_step_##P##_2(bool noise, bool zbc, int vec);                                                    \
-    int occupancy_step_##P##_3(bool noise, bool zbc, int vec);
+    cudaError_t launch_step_##P##_0(const StepArgs<T>&, bool noise, bool zbc, bool iso, int vec, dim3 grid, cudaStream_t); \
+    cudaError_t launch_step_##P##_1(const StepArgs<T>&, bool noise, bool zbc, bool iso, int vec, dim3 grid, cudaStream_t); \
+    cudaError_t launch_step_##P##_2(const StepArgs<T>&, bool noise, bool zbc, bool iso, int vec, dim3 grid, cudaStream_t); \
+    cudaError_t launch_step_##P##_3(const StepArgs<T>&, bool noise, bool zbc, bool iso, int vec, dim3 grid, cudaStream_t); \
+    int occupancy_step_##P##_0(bool noise, bool zbc, bool iso, int vec);                                          \
+    int occupancy_step_##P##_1(bool noise, bool zbc, bool iso, int vec);                                          \
+    int occupancy_step_##P##_2(bool noise, bool zbc, bool iso, int vec);                                          \
+    int occupancy_step_##P##_3(bool noise, bool zbc, bool iso, int vec);
 PHX_DECL_STEP(32, float)
 PHX_DECL_STEP(64, double)
 #undef PHX_DECL_STEP

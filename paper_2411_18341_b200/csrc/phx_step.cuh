@@ -21,12 +21,13 @@
 #include "phx_common.cuh"
 #include "phx_deriv.cuh"
 #include "phx_philox.cuh"
+#include "phx_launch.h"
 
 #ifndef PHX_STEP_UNROLL
 #define PHX_STEP_UNROLL 4
 #endif
 #ifndef PHX_STEP_PF_ROWS
-#define PHX_STEP_PF_ROWS 6
+#define PHX_STEP_PF_ROWS 4
 #endif
 
 namespace phx {
@@ -131,8 +132,9 @@ __device__ __forceinline__ void gather(const typename Cx<T>::type (&rs)[VEC], co
 // register either).  RING = 5 is the longest life: psi rows j-2 .. j+2 and V rows j-3 .. j+1.
 #define PHX_STEP_RING 5
 
-template <typename T, int VEC, int MODEL, bool NOISE, bool ZBC, int MINB>
-__global__ void __launch_bounds__(128, MINB)
+// MINW: resident warps per SM the register budget is sized for.  ISO: dx == dy (scalar and reservoir models only).
+template <typename T, int VEC, int MODEL, bool NOISE, bool ZBC, bool ISO, int MINW>
+__global__ void __launch_bounds__(32 * PHX_STEP_WARPS, MINW / PHX_STEP_WARPS)
 step_kernel(const __grid_constant__ StepArgs<T> a) {
     using namespace stepk;
     using C = typename Cx<T>::type;
@@ -146,7 +148,7 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
     const int nx = g.nx, ny = g.ny;
 
     const int lane = threadIdx.x & 31;
-    const int strip = blockIdx.x * 4 + (threadIdx.x >> 5);
+    const int strip = blockIdx.x * PHX_STEP_WARPS + (threadIdx.x >> 5);
     const uint64_t step = *a.step_in;
     if (blockIdx.x == 0 && blockIdx.y == 0 && blockIdx.z == 0 && threadIdx.x == 0) *a.step_out = step + 1;
     if (strip >= a.strips) return;   // warp-uniform
@@ -337,11 +339,11 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
                 Nbhd<T> nb[NC][VEC];
                 Diff<T> df[NC][VEC];
                 auto O = [](int s) { return SPINOR ? 1 - s : 0; };            // index of the other component
-                auto diffs = [](const Nbhd<T> (&nb)[NC][VEC], Diff<T> (&df)[NC][VEC]) {
+                auto diffs = [&k](const Nbhd<T> (&nb)[NC][VEC], Diff<T> (&df)[NC][VEC]) {
 #pragma unroll
                     for (int s = 0; s < NC; ++s) {
 #pragma unroll
-                        for (int i = 0; i < VEC; ++i) differences<T, SPINOR>(nb[s][i], df[s][i]);
+                        for (int i = 0; i < VEC; ++i) differences<T, SPINOR, ISO>(k, nb[s][i], df[s][i]);
                     }
                 };
 

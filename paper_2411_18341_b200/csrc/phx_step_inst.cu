@@ -15,68 +15,79 @@ typedef float real_t;
 typedef double real_t;
 #endif
 
-// Resident CTAs (of 4 warps) per SM the register budget is sized for: the carried register windows grow with the
-// number of components and reservoirs (DESIGN.md section 5.2 has the count per model).
+// Resident warps per SM the register budget is sized for: the carried register rings grow with the number of
+// components and reservoirs (DESIGN.md section 5.2 has the count per model).
 #if PHX_INST_PREC == 32
-#ifndef PHX_MINB_V2
-#define PHX_MINB_V2 (PHX_INST_MODEL == 0 ? 4 : (PHX_INST_MODEL == 1 ? 3 : 2))
+#ifndef PHX_MINW_V2
+#define PHX_MINW_V2 (PHX_INST_MODEL == 0 ? 16 : (PHX_INST_MODEL == 1 ? 12 : 8))
 #endif
-#define PHX_MINB_V1 (PHX_INST_MODEL == 0 ? 6 : (PHX_INST_MODEL == 1 ? 5 : 3))
+#define PHX_MINW_V1 (PHX_INST_MODEL == 0 ? 24 : (PHX_INST_MODEL == 1 ? 20 : 12))
 #else
-#define PHX_MINB_V2 2
-#define PHX_MINB_V1 (PHX_INST_MODEL == 0 ? 4 : (PHX_INST_MODEL == 1 ? 3 : 2))
+#define PHX_MINW_V2 8
+#define PHX_MINW_V1 (PHX_INST_MODEL == 0 ? 16 : (PHX_INST_MODEL == 1 ? 12 : 8))
 #endif
+// The isotropic form of the Laplacian exists for the models without TE-TM coupling.
+#define PHX_HAS_ISO (PHX_INST_MODEL < 2)
 
-template <int VEC, bool NOISE, bool ZBC>
-static cudaError_t launch_one(const StepArgs<real_t>& a, dim3 grid, cudaStream_t st) {
-    constexpr int MINB = VEC == 2 ? PHX_MINB_V2 : PHX_MINB_V1;
-    step_kernel<real_t, VEC, PHX_INST_MODEL, NOISE, ZBC, MINB><<<grid, 128, 0, st>>>(a);
-    return cudaGetLastError();
-}
-
-template <int VEC, bool NOISE, bool ZBC>
-static int occ_one() {
-    constexpr int MINB = VEC == 2 ? PHX_MINB_V2 : PHX_MINB_V1;
-    int nb = 0;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, step_kernel<real_t, VEC, PHX_INST_MODEL, NOISE, ZBC, MINB>, 128, 0) != cudaSuccess) {
-        cudaGetLastError();
-        return MINB;
+template <int VEC, bool NOISE, bool ZBC, bool ISO>
+struct Inst {
+    static constexpr int MINW = VEC == 2 ? PHX_MINW_V2 : PHX_MINW_V1;
+    static constexpr bool I = ISO && PHX_HAS_ISO;
+    static cudaError_t launch(const StepArgs<real_t>& a, dim3 grid, cudaStream_t st) {
+        step_kernel<real_t, VEC, PHX_INST_MODEL, NOISE, ZBC, I, MINW><<<grid, 32 * PHX_STEP_WARPS, 0, st>>>(a);
+        return cudaGetLastError();
     }
-    return nb;
+    static int occupancy() {   // resident CTAs per SM
+        int nb = 0;
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, step_kernel<real_t, VEC, PHX_INST_MODEL, NOISE, ZBC, I, MINW>,
+                                                          32 * PHX_STEP_WARPS, 0) != cudaSuccess) {
+            cudaGetLastError();
+            return MINW / PHX_STEP_WARPS;
+        }
+        return nb;
+    }
+};
+
+template <int VEC, typename F>
+static auto dispatch(bool noise, bool zbc, bool iso, F f) {
+    if (noise) {
+        if (zbc) return iso ? f(Inst<VEC, true, true, true>()) : f(Inst<VEC, true, true, false>());
+        return iso ? f(Inst<VEC, true, false, true>()) : f(Inst<VEC, true, false, false>());
+    }
+    if (zbc) return iso ? f(Inst<VEC, false, true, true>()) : f(Inst<VEC, false, true, false>());
+    return iso ? f(Inst<VEC, false, false, true>()) : f(Inst<VEC, false, false, false>());
 }
 
 template <int VEC>
-static int occ_vec(bool noise, bool zbc) {
-    if (noise) return zbc ? occ_one<VEC, true, true>() : occ_one<VEC, true, false>();
-    return zbc ? occ_one<VEC, false, true>() : occ_one<VEC, false, false>();
+static int occ_vec(bool noise, bool zbc, bool iso) {
+    return dispatch<VEC>(noise, zbc, iso, [](auto inst) { return decltype(inst)::occupancy(); });
 }
 
 template <int VEC>
-static cudaError_t launch_vec(const StepArgs<real_t>& a, bool noise, bool zbc, dim3 grid, cudaStream_t st) {
-    if (noise) return zbc ? launch_one<VEC, true, true>(a, grid, st) : launch_one<VEC, true, false>(a, grid, st);
-    return zbc ? launch_one<VEC, false, true>(a, grid, st) : launch_one<VEC, false, false>(a, grid, st);
+static cudaError_t launch_vec(const StepArgs<real_t>& a, bool noise, bool zbc, bool iso, dim3 grid, cudaStream_t st) {
+    return dispatch<VEC>(noise, zbc, iso, [&](auto inst) { return decltype(inst)::launch(a, grid, st); });
 }
 
 #define PHX_CAT3(a, b, c) a##b##_##c
 #define PHX_NAME(p, m) PHX_CAT3(launch_step_, p, m)
 
-cudaError_t PHX_NAME(PHX_INST_PREC, PHX_INST_MODEL)(const StepArgs<real_t>& a, bool noise, bool zbc, int vec, dim3 grid,
-                                                    cudaStream_t st) {
+cudaError_t PHX_NAME(PHX_INST_PREC, PHX_INST_MODEL)(const StepArgs<real_t>& a, bool noise, bool zbc, bool iso, int vec,
+                                                    dim3 grid, cudaStream_t st) {
 #if PHX_INST_PREC == 32
-    if (vec == 2) return launch_vec<2>(a, noise, zbc, grid, st);
+    if (vec == 2) return launch_vec<2>(a, noise, zbc, iso, grid, st);
 #endif
-    if (vec == 1) return launch_vec<1>(a, noise, zbc, grid, st);
+    if (vec == 1) return launch_vec<1>(a, noise, zbc, iso, grid, st);
     return cudaErrorInvalidValue;
 }
 
 #define PHX_OCC_NAME(p, m) PHX_CAT3(occupancy_step_, p, m)
 
 // Resident CTAs per SM of the instantiation (for the launch plan: one balanced wave).
-int PHX_OCC_NAME(PHX_INST_PREC, PHX_INST_MODEL)(bool noise, bool zbc, int vec) {
+int PHX_OCC_NAME(PHX_INST_PREC, PHX_INST_MODEL)(bool noise, bool zbc, bool iso, int vec) {
 #if PHX_INST_PREC == 32
-    if (vec == 2) return occ_vec<2>(noise, zbc);
+    if (vec == 2) return occ_vec<2>(noise, zbc, iso);
 #endif
-    return occ_vec<1>(noise, zbc);
+    return occ_vec<1>(noise, zbc, iso);
 }
 
 }  // namespace phx

@@ -32,10 +32,11 @@ __device__ __forceinline__ double2 fma2s(double s, double2 a, double2 c) { retur
 __device__ __forceinline__ float2 rot(float2 a) { return make_float2(-a.y, a.x); }
 __device__ __forceinline__ double2 rot(double2 a) { return make_double2(-a.y, a.x); }
 
-// Nine-point neighbourhood of one component around a cell.  Scalar models read only c, w, e, s, n.
+// Neighbourhood of one component around a cell: the five points of Eq. (8) and, for the TE-TM operator, the
+// undivided corner difference D = Dxy4 = (n - s)[east column] - (n - s)[west column] (set by the spinor models only).
 template <typename T>
 struct Nbhd {
-    typename Cx<T>::type c, w, e, s, n, sw, se, nw, ne;   // s = row j-1, n = row j+1, w = column i-1, e = column i+1
+    typename Cx<T>::type c, w, e, s, n, D;   // s = row j-1, n = row j+1, w = column i-1, e = column i+1
 };
 
 // Differences of one component at a cell: L = (hbar/2m) lap, Eq. (8); for the TE-TM operator also the undivided
@@ -56,7 +57,7 @@ __device__ __forceinline__ void differences(const Coef<T>& k, const Nbhd<T>& nb,
         d.B = fma2s(T(-2), nb.c, add2(nb.n, nb.s));
         d.L = fma2s(k.cy, d.B, mul2s(k.cx, d.A));
     }
-    if (NINE) d.D = add2(sub2(nb.ne, nb.se), sub2(nb.sw, nb.nw));
+    if (NINE) d.D = nb.D;
 }
 
 // K = i L - i W y + (Rr n / 2 - hgc) y - i J[other],  Kn = P - (gamr + Rr rho) n

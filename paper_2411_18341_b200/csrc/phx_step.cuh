@@ -94,33 +94,30 @@ __device__ __forceinline__ double2 up1(double2 v) { return make_double2(__shfl_u
 __device__ __forceinline__ double2 dn1(double2 v) { return make_double2(__shfl_down_sync(0xffffffffu, v.x, 1), __shfl_down_sync(0xffffffffu, v.y, 1)); }
 
 // Neighbourhood of cell i of the centre row (rc) of a three-row window (rs = row below, rn = row above);
-// west/east of the lane's cells by shuffle.  NINE = false leaves the corners unset (scalar models never read them).
+// west/east of the lane's cells by shuffle.  NINE (spinor models): the corner difference Dxy4 is formed from the
+// vertical differences n - s of the neighbouring columns, so that one pair per side crosses lanes instead of two.
 template <typename T, int VEC, bool NINE>
 __device__ __forceinline__ void gather(const typename Cx<T>::type (&rs)[VEC], const typename Cx<T>::type (&rc)[VEC],
                                        const typename Cx<T>::type (&rn)[VEC], Nbhd<T> (&nb)[VEC]) {
     using C = typename Cx<T>::type;
-    C west[3], east[3];
-    west[1] = up1(rc[VEC - 1]);
-    east[1] = dn1(rc[0]);
-    if (NINE) {
-        west[0] = up1(rs[VEC - 1]);
-        east[0] = dn1(rs[0]);
-        west[2] = up1(rn[VEC - 1]);
-        east[2] = dn1(rn[0]);
-    }
+    const C west = up1(rc[VEC - 1]);
+    const C east = dn1(rc[0]);
 #pragma unroll
     for (int i = 0; i < VEC; ++i) {
         nb[i].c = rc[i];
         nb[i].s = rs[i];
         nb[i].n = rn[i];
-        nb[i].w = i == 0 ? west[1] : rc[i - 1];
-        nb[i].e = i == VEC - 1 ? east[1] : rc[i + 1];
-        if (NINE) {
-            nb[i].sw = i == 0 ? west[0] : rs[i - 1];
-            nb[i].se = i == VEC - 1 ? east[0] : rs[i + 1];
-            nb[i].nw = i == 0 ? west[2] : rn[i - 1];
-            nb[i].ne = i == VEC - 1 ? east[2] : rn[i + 1];
-        }
+        nb[i].w = i == 0 ? west : rc[i - 1];
+        nb[i].e = i == VEC - 1 ? east : rc[i + 1];
+    }
+    if (NINE) {
+        C vd[VEC];
+#pragma unroll
+        for (int i = 0; i < VEC; ++i) vd[i] = sub2(rn[i], rs[i]);
+        const C vwest = up1(vd[VEC - 1]);
+        const C veast = dn1(vd[0]);
+#pragma unroll
+        for (int i = 0; i < VEC; ++i) nb[i].D = sub2(i == VEC - 1 ? veast : vd[i + 1], i == 0 ? vwest : vd[i - 1]);
     }
 }
 

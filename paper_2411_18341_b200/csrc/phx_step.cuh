@@ -53,23 +53,32 @@ struct StepArgs {
 namespace stepk {
 
 template <int VEC> __device__ __forceinline__ void ldc(const float2* p, float2 (&v)[VEC]) {
-    if constexpr (VEC == 2) { const float4 q = __ldg(reinterpret_cast<const float4*>(p)); v[0] = make_float2(q.x, q.y); v[1] = make_float2(q.z, q.w); }
-    else v[0] = __ldg(p);
+    if constexpr (VEC % 2 == 0) {
+#pragma unroll
+        for (int h = 0; h < VEC / 2; ++h) {
+            const float4 q = __ldg(reinterpret_cast<const float4*>(p) + h);
+            v[2 * h] = make_float2(q.x, q.y);
+            v[2 * h + 1] = make_float2(q.z, q.w);
+        }
+    } else v[0] = __ldg(p);
 }
 template <int VEC> __device__ __forceinline__ void ldc(const double2* p, double2 (&v)[VEC]) {
 #pragma unroll
     for (int i = 0; i < VEC; ++i) v[i] = __ldg(p + i);
 }
 template <int VEC> __device__ __forceinline__ void stc(float2* p, const float2 (&v)[VEC]) {
-    if constexpr (VEC == 2) *reinterpret_cast<float4*>(p) = make_float4(v[0].x, v[0].y, v[1].x, v[1].y);
-    else *p = v[0];
+    if constexpr (VEC % 2 == 0) {
+#pragma unroll
+        for (int h = 0; h < VEC / 2; ++h) reinterpret_cast<float4*>(p)[h] = make_float4(v[2 * h].x, v[2 * h].y, v[2 * h + 1].x, v[2 * h + 1].y);
+    } else *p = v[0];
 }
 template <int VEC> __device__ __forceinline__ void stc(double2* p, const double2 (&v)[VEC]) {
 #pragma unroll
     for (int i = 0; i < VEC; ++i) p[i] = v[i];
 }
 template <int VEC> __device__ __forceinline__ void ldr(const float* p, float (&v)[VEC]) {
-    if constexpr (VEC == 2) { const float2 q = __ldg(reinterpret_cast<const float2*>(p)); v[0] = q.x; v[1] = q.y; }
+    if constexpr (VEC == 4) { const float4 q = __ldg(reinterpret_cast<const float4*>(p)); v[0] = q.x; v[1] = q.y; v[2] = q.z; v[3] = q.w; }
+    else if constexpr (VEC == 2) { const float2 q = __ldg(reinterpret_cast<const float2*>(p)); v[0] = q.x; v[1] = q.y; }
     else v[0] = __ldg(p);
 }
 template <int VEC> __device__ __forceinline__ void ldr(const double* p, double (&v)[VEC]) {
@@ -77,7 +86,8 @@ template <int VEC> __device__ __forceinline__ void ldr(const double* p, double (
     else v[0] = __ldg(p);
 }
 template <int VEC> __device__ __forceinline__ void str(float* p, const float (&v)[VEC]) {
-    if constexpr (VEC == 2) *reinterpret_cast<float2*>(p) = make_float2(v[0], v[1]);
+    if constexpr (VEC == 4) *reinterpret_cast<float4*>(p) = make_float4(v[0], v[1], v[2], v[3]);
+    else if constexpr (VEC == 2) *reinterpret_cast<float2*>(p) = make_float2(v[0], v[1]);
     else *p = v[0];
 }
 template <int VEC> __device__ __forceinline__ void str(double* p, const double (&v)[VEC]) {

@@ -28,10 +28,14 @@ typedef double real_t;
 #endif
 // The isotropic form of the Laplacian exists for the models without TE-TM coupling.
 #define PHX_HAS_ISO (PHX_INST_MODEL < 2)
+// Four cells per lane (two 128-bit loads): complex fp32, scalar model only (the other models run out of registers).
+#ifndef PHX_HAS_VEC4
+#define PHX_HAS_VEC4 (PHX_INST_PREC == 32 && PHX_INST_MODEL == 0)
+#endif
 
 template <int VEC, bool NOISE, bool ZBC, bool ISO>
 struct Inst {
-    static constexpr int MINW = VEC == 2 ? PHX_MINW_V2 : PHX_MINW_V1;
+    static constexpr int MINW = VEC == 4 ? 8 : (VEC == 2 ? PHX_MINW_V2 : PHX_MINW_V1);
     static constexpr bool I = ISO && PHX_HAS_ISO;
     static cudaError_t launch(const StepArgs<real_t>& a, dim3 grid, cudaStream_t st) {
         step_kernel<real_t, VEC, PHX_INST_MODEL, NOISE, ZBC, I, MINW><<<grid, 32 * PHX_STEP_WARPS, 0, st>>>(a);
@@ -74,6 +78,9 @@ static cudaError_t launch_vec(const StepArgs<real_t>& a, bool noise, bool zbc, b
 cudaError_t PHX_NAME(PHX_INST_PREC, PHX_INST_MODEL)(const StepArgs<real_t>& a, bool noise, bool zbc, bool iso, int vec,
                                                     dim3 grid, cudaStream_t st) {
 #if PHX_INST_PREC == 32
+#if PHX_HAS_VEC4
+    if (vec == 4) return launch_vec<4>(a, noise, zbc, iso, grid, st);
+#endif
     if (vec == 2) return launch_vec<2>(a, noise, zbc, iso, grid, st);
 #endif
     if (vec == 1) return launch_vec<1>(a, noise, zbc, iso, grid, st);
@@ -85,6 +92,9 @@ cudaError_t PHX_NAME(PHX_INST_PREC, PHX_INST_MODEL)(const StepArgs<real_t>& a, b
 // Resident CTAs per SM of the instantiation (for the launch plan: one balanced wave).
 int PHX_OCC_NAME(PHX_INST_PREC, PHX_INST_MODEL)(bool noise, bool zbc, bool iso, int vec) {
 #if PHX_INST_PREC == 32
+#if PHX_HAS_VEC4
+    if (vec == 4) return occ_vec<4>(noise, zbc, iso);
+#endif
     if (vec == 2) return occ_vec<2>(noise, zbc, iso);
 #endif
     return occ_vec<1>(noise, zbc, iso);

@@ -2,6 +2,8 @@
 section 5.2) against the CPU oracle, element by element, plus the invariants that need no oracle.
 Bars as in test_gpu_parity.py (BASELINE.json north_star): relative L2 <= 1e-12 (complex fp64), <= 2e-5 (complex fp32).
 Sizes span several warp strips (56 / 24 output columns per strip) and row chunks with ragged tails in x and y."""
+import dataclasses
+
 import numpy as np
 import pytest
 
@@ -38,10 +40,33 @@ def test_cfg2_reduced(prec, nx, ny):
     run_pair(w, 101)                               # odd count: the state ends in the alternate buffer
 
 
-@pytest.mark.parametrize("tuning", [{"step_ly": 8}, {"step_ly": 13, "step_vec": 1}, {"step_ly": 1000}])
+@pytest.mark.parametrize("tuning", [{"step_ly": 8}, {"step_ly": 13, "step_vec": 1}, {"step_ly": 1000},
+                                    {"step_ly": 13, "step_vec": 4}, {"step_vec": 4}])
 def test_cfg2_chunking(tuning):
     w = wl.cfg2(n=300, ny=70, prec="c32")
     run_pair(w, 60, tuning=tuning)
+
+
+@pytest.mark.parametrize("prec", ["c32", "c64"])
+@pytest.mark.parametrize("model", ["scalar", "reservoir", "spinor_reservoir"])
+def test_anisotropic_grid(prec, model):
+    # dx != dy: the general form of the Laplacian (cx != cy); every other STEP case here has dx == dy
+    w = {"scalar": lambda: wl.cfg2(n=300, ny=70, prec=prec), "reservoir": lambda: wl.cfg3(n=96, prec=prec),
+         "spinor_reservoir": lambda: wl.example3(n=90, prec=prec)}[model]()
+    w = dataclasses.replace(w, dy=w.dx * 1.25)
+    run_pair(w, 60)
+    if model == "scalar" and prec == "c32":
+        run_pair(w, 60, tuning={"step_vec": 4})
+
+
+def test_wide_scalar_grid_takes_four_cells_per_lane():
+    w = wl.cfg2(n=2048, ny=48, prec="c32")
+    g = make_gpu(w, variant=STEP)
+    o = make_oracle(w)
+    g.step_rk4(30)
+    o.step_rk4(30)
+    compare(g, o, w)
+    g.destroy()
 
 
 @pytest.mark.parametrize("prec", ["c32", "c64"])
@@ -76,9 +101,10 @@ def test_zero_boundaries(bc, model):
     run_pair(w, 50, bc=bc)
 
 
-def test_zero_boundaries_fp32_two_cells_per_lane():
-    w = wl.cfg2(n=130, ny=70, prec="c32")
-    run_pair(w, 50, bc=(1, 1), tuning={"step_ly": 16})
+@pytest.mark.parametrize("vec", [2, 4])
+def test_zero_boundaries_fp32_cells_per_lane(vec):
+    w = wl.cfg2(n=132, ny=70, prec="c32")
+    run_pair(w, 50, bc=(1, 1), tuning={"step_ly": 16, "step_vec": vec})
 
 
 def test_density_offset():
@@ -161,6 +187,12 @@ def test_shift_equivariance_bit_exact(model):
     for k in w.fields:
         assert np.array_equal(np.roll(base[k], sh, (1, 2)), g2.read_field(k)), k
     g2.destroy()
+    if model == "scalar":   # four cells per lane: the same arithmetic per cell, so the same bits
+        g4 = make_gpu(w2, variant=STEP, tuning={"step_vec": 4})
+        g4.step_rk4(10)
+        for k in w.fields:
+            assert np.array_equal(np.roll(base[k], sh, (1, 2)), g4.read_field(k)), k
+        g4.destroy()
 
 
 def test_step_splitting_and_checkpoint_are_bit_exact_with_noise():

@@ -147,6 +147,22 @@ def measured_peaks():
     return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
+def max_over_ranks(x, world, device="cuda"):
+    """A time is the slowest rank's (the contract: device time, max over ranks)."""
+    if world <= 1:
+        return float(x)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([float(x)], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(world, cells, steps, ms):
+    """Replicas only: every rank steps its own copy, the job's cell-steps add up."""
+    return world * cells * steps / (ms * 1e-3) / 1e9
+
+
 def oracle_from_workload(w, ny=None):
     """The oracle as it stands on (a row-slab sample of) the workload."""
     import oracle as orc
@@ -243,11 +259,7 @@ def main():
         g.step_rk4(steps)
         e1.record(stream)
         barrier()
-        t_ms = e0.elapsed_time(e1)
-        if world > 1:
-            t = torch.tensor([t_ms], device="cuda")
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            t_ms = float(t.item())
+        t_ms = max_over_ranks(e0.elapsed_time(e1), world)
         return t_ms, g.get_launch_count() - launches0
 
     g.step_rk4(args.warmup)
@@ -261,7 +273,7 @@ def main():
     t_wall1 = time.time()
     clocks = sampler.stop(t_wall0, t_wall1) if rank == 0 else None
     cells = w.cells
-    value = world * cells * args.steps / (ms * 1e-3) / 1e9
+    value = whole_job_value(world, cells, args.steps, ms)
 
     # the per-stage variant (the HBM-bound kernels of the north_star's >= 70 % target), timed the same way on a
     # shorter run, when the headline ran the fused step
@@ -272,7 +284,7 @@ def main():
         st_steps = max(8, args.steps // 4)
         st_ms, st_launches = timed(st_steps)
         st_bpc = algo_bytes_per_cell_step(w, phx.PHX_VARIANT_STAGE)
-        st_val = world * cells * st_steps / (st_ms * 1e-3) / 1e9
+        st_val = whole_job_value(world, cells, st_steps, st_ms)
         st_gbs = st_bpc * cells * st_steps / (st_ms * 1e-3) / 1e9
         stage_info = {"variant": 1, "kernel": "phx::stage_kernel (4 launches per step)", "value": st_val, "unit": UNIT,
                       "steps": st_steps, "ms_per_step": st_ms / st_steps, "gpu_launches": int(st_launches),
@@ -300,12 +312,8 @@ def main():
     for _ in range(args.e2e_steps):
         e2e_step()
     barrier()
-    e2e_s = time.perf_counter() - t0
-    if world > 1:
-        t = torch.tensor([e2e_s], device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_s = float(t.item())
-    e2e_val = world * cells * args.e2e_steps / e2e_s / 1e9
+    e2e_s = max_over_ranks(time.perf_counter() - t0, world)
+    e2e_val = whole_job_value(world, cells, args.e2e_steps, e2e_s * 1e3)
 
     if rank != 0:
         if world > 1:

@@ -28,9 +28,6 @@ def _units():
                       [f"-DPHX_INST_PREC={prec}", f"-DPHX_INST_MODEL={model}"]))
             u.append((f"phx_step_{prec}_{model}.o", "phx_step_inst.cu",
                       [f"-DPHX_INST_PREC={prec}", f"-DPHX_INST_MODEL={model}"]))
-    for extra in ("phx_resident.cu",):
-        if os.path.exists(os.path.join(CSRC, extra)):
-            u.append((extra.replace(".cu", ".o"), extra, []))
     return u
 
 

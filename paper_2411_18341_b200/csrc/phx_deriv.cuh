@@ -2,7 +2,7 @@
 // one component: five-point Laplacian Eq. (8); local terms of Eq. (1)/(16) PAPER.md:25, :361
 // (sign and form as Listing 2); reservoir Eq. (17); compact nine-point TE-TM
 // operator Delta_LT (d_x -+ i d_y)^2 on the other component.
-// Used by the temporally blocked variants (STEP, RESIDENT).  Product code: shares nothing with oracle/.
+// Used by the temporally blocked variant STEP.  Product code: shares nothing with oracle/.
 //
 // Written on (re, im) PAIRS: for complex fp32 every pair operation below is one packed sm_100 instruction
 // (FADD2 / FMUL2 / FFMA2 on a 64-bit register pair), and multiplication by +-i is an operand modifier of that

@@ -23,9 +23,6 @@
 #include "phx_philox.cuh"
 #include "phx_launch.h"
 
-#ifndef PHX_STEP_UNROLL
-#define PHX_STEP_UNROLL 4
-#endif
 #ifndef PHX_STEP_PF_ROWS
 #define PHX_STEP_PF_ROWS 4
 #endif

@@ -234,7 +234,9 @@ cudaError_t enqueue_step_stage(phx_grid* g, cudaStream_t st) {
 // ---- variant STEP: launch plan ---------------------------------------------------------------------------------
 int step_vec(const phx_grid* g) {
     if (g->step_vec) return g->step_vec;
-    if (g->d.prec != PHX_C32 || g->d.nx % 2 != 0) return 1;
+    if (g->d.nx % 2 != 0) return 1;
+    // complex fp64: two cells per lane (strips of 64 columns, 56 output columns instead of 24 of 32) on wide scalar grids
+    if (g->d.prec != PHX_C32) return (g->d.model == PHX_SCALAR && g->d.nx >= 1024) ? 2 : 1;
     // four cells per lane: strips of 128 columns (120 output columns), 8 resident warps per SM; pays on wide scalar grids
     if (g->d.model == PHX_SCALAR && g->d.nx % 4 == 0 && g->d.nx >= 2048) return 4;
     return 2;
@@ -682,8 +684,9 @@ phx_status phx_set_tuning(phx_grid* g, const char* key, int32_t value) {
         g->step_ly = value;
     } else if (!std::strcmp(key, "step_vec")) {       // variant STEP: cells per lane (0 = automatic)
         if (value != 0 && value != 1 && value != 2 && value != 4) return PHX_ERR_INVALID_ARG;
-        if (value >= 2 && (g->d.nx % value != 0 || g->d.prec != PHX_C32)) return fail(g, PHX_ERR_UNSUPPORTED, "step_vec>1 needs complex fp32 and nx a multiple of it");
-        if (value == 4 && g->d.model != PHX_SCALAR) return fail(g, PHX_ERR_UNSUPPORTED, "step_vec=4 exists for the scalar model only");
+        if (value >= 2 && g->d.nx % value != 0) return fail(g, PHX_ERR_UNSUPPORTED, "step_vec>1 needs nx a multiple of it");
+        if (value == 4 && (g->d.model != PHX_SCALAR || g->d.prec != PHX_C32)) return fail(g, PHX_ERR_UNSUPPORTED, "step_vec=4 exists for the scalar fp32 model only");
+        if (value == 2 && g->d.prec == PHX_C64 && g->d.model != PHX_SCALAR) return fail(g, PHX_ERR_UNSUPPORTED, "step_vec=2 in fp64 exists for the scalar model only");
         g->step_vec = value;
     } else if (!std::strcmp(key, "graph_steps")) {
         if (value < 1 || value > 256) return PHX_ERR_INVALID_ARG;

@@ -29,6 +29,10 @@ typedef double real_t;
 // The isotropic form of the Laplacian exists for the models without TE-TM coupling.
 #define PHX_HAS_ISO (PHX_INST_MODEL < 2)
 // Four cells per lane (two 128-bit loads): complex fp32, scalar model only (the other models run out of registers).
+// Two cells per lane in complex fp64 (two 128-bit loads), scalar model only.
+#ifndef PHX_HAS_VEC2_64
+#define PHX_HAS_VEC2_64 (PHX_INST_PREC == 64 && PHX_INST_MODEL == 0)
+#endif
 #ifndef PHX_HAS_VEC4
 #define PHX_HAS_VEC4 (PHX_INST_PREC == 32 && PHX_INST_MODEL == 0)
 #endif
@@ -82,6 +86,8 @@ cudaError_t PHX_NAME(PHX_INST_PREC, PHX_INST_MODEL)(const StepArgs<real_t>& a, b
     if (vec == 4) return launch_vec<4>(a, noise, zbc, iso, grid, st);
 #endif
     if (vec == 2) return launch_vec<2>(a, noise, zbc, iso, grid, st);
+#elif PHX_HAS_VEC2_64
+    if (vec == 2) return launch_vec<2>(a, noise, zbc, iso, grid, st);
 #endif
     if (vec == 1) return launch_vec<1>(a, noise, zbc, iso, grid, st);
     return cudaErrorInvalidValue;
@@ -95,6 +101,8 @@ int PHX_OCC_NAME(PHX_INST_PREC, PHX_INST_MODEL)(bool noise, bool zbc, bool iso, 
 #if PHX_HAS_VEC4
     if (vec == 4) return occ_vec<4>(noise, zbc, iso);
 #endif
+    if (vec == 2) return occ_vec<2>(noise, zbc, iso);
+#elif PHX_HAS_VEC2_64
     if (vec == 2) return occ_vec<2>(noise, zbc, iso);
 #endif
     return occ_vec<1>(noise, zbc, iso);

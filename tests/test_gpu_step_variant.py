@@ -59,6 +59,14 @@ def test_anisotropic_grid(prec, model):
         run_pair(w, 60, tuning={"step_vec": 4})
 
 
+@pytest.mark.parametrize("tuning", [{"step_vec": 2}, {"step_vec": 2, "step_ly": 11}])
+def test_cfg2_fp64_two_cells_per_lane(tuning):
+    w = wl.cfg2(n=300, ny=70, prec="c64")
+    run_pair(w, 60, tuning=tuning)
+    run_pair(dataclasses.replace(w, dy=w.dx * 0.8), 40, tuning=tuning)      # general (dx != dy) form
+    run_pair(wl.cfg2(n=132, ny=70, prec="c64"), 40, bc=(1, 1), tuning=tuning)   # zero boundaries
+
+
 def test_wide_scalar_grid_takes_four_cells_per_lane():
     w = wl.cfg2(n=2048, ny=48, prec="c32")
     g = make_gpu(w, variant=STEP)

@@ -61,10 +61,10 @@ typedef enum { PHX_BC_PERIODIC = 0, PHX_BC_ZERO = 1 } phx_boundary;   /* PAPER.m
 
 /* Kernel variants (all compute the same RK4 step; they differ in how often data crosses HBM). */
 typedef enum {
-    PHX_VARIANT_AUTO = 0,      /* the fastest variant that can run the grid: STEP, or STAGE when a drive is set */
+    PHX_VARIANT_AUTO = 0,      /* the fastest variant that can run the grid: STEP, or STAGE for a driven grid with noise */
     PHX_VARIANT_STAGE = 1,     /* one fused kernel per RK stage (4 launches per step); every model and term */
     PHX_VARIANT_STEP = 3,      /* one kernel per RK4 step: the four stages pipelined along y in register windows of
-                                  a haloed warp-wide column strip (N_halo = 4); no drive term */
+                                  a haloed warp-wide column strip (N_halo = 4); not for drive + noise together */
     PHX_VARIANT_RESIDENT = 4   /* whole grid resident on chip, many steps per launch (small grids) */
 } phx_variant;
 

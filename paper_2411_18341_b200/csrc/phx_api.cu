@@ -246,20 +246,20 @@ int step_vec(const phx_grid* g) {
 bool step_iso(const phx_grid* g) { return g->d.dx == g->d.dy; }
 
 int step_occupancy(const phx_grid* g, int vec) {
-    const bool noise = g->d.noise != 0, zbc = g->d.bc_x || g->d.bc_y, iso = step_iso(g);
+    const bool noise = g->d.noise != 0, zbc = g->d.bc_x || g->d.bc_y, iso = step_iso(g), drive = g->hasE;
     if (g->d.prec == PHX_C32) {
         switch (g->d.model) {
-            case 0: return occupancy_step_32_0(noise, zbc, iso, vec);
-            case 1: return occupancy_step_32_1(noise, zbc, iso, vec);
-            case 2: return occupancy_step_32_2(noise, zbc, iso, vec);
-            default: return occupancy_step_32_3(noise, zbc, iso, vec);
+            case 0: return occupancy_step_32_0(noise, zbc, iso, drive, vec);
+            case 1: return occupancy_step_32_1(noise, zbc, iso, drive, vec);
+            case 2: return occupancy_step_32_2(noise, zbc, iso, drive, vec);
+            default: return occupancy_step_32_3(noise, zbc, iso, drive, vec);
         }
     }
     switch (g->d.model) {
-        case 0: return occupancy_step_64_0(noise, zbc, iso, vec);
-        case 1: return occupancy_step_64_1(noise, zbc, iso, vec);
-        case 2: return occupancy_step_64_2(noise, zbc, iso, vec);
-        default: return occupancy_step_64_3(noise, zbc, iso, vec);
+        case 0: return occupancy_step_64_0(noise, zbc, iso, drive, vec);
+        case 1: return occupancy_step_64_1(noise, zbc, iso, drive, vec);
+        case 2: return occupancy_step_64_2(noise, zbc, iso, drive, vec);
+        default: return occupancy_step_64_3(noise, zbc, iso, drive, vec);
     }
 }
 
@@ -307,6 +307,7 @@ cudaError_t enqueue_step_fused(phx_grid* g, cudaStream_t st, int parity) {
     }
     a.V = g->hasV ? (const T*)(g->ws + g->L.V) : nullptr;
     a.P = g->hasP ? (const T*)(g->ws + g->L.P) : nullptr;
+    a.E = g->hasE ? (const C*)(g->ws + g->L.E) : nullptr;
     uint64_t* slots = (uint64_t*)(g->ws + g->L.step);
     a.step_in = slots + parity;
     a.step_out = slots + (1 - parity);
@@ -360,8 +361,10 @@ cudaError_t capture(phx_grid* g, int steps, int parity, cudaGraphExec_t* out) {
     return e;
 }
 
-// The fused step carries no drive term, and addresses a plane by 32-bit cell offsets.
-bool step_variant_ok(const phx_grid* g) { return !g->hasE && (size_t)g->d.nx * (size_t)g->d.ny < ((size_t)1 << 31); }
+// The fused step addresses a plane by 32-bit cell offsets; its driven kernels are built without noise.
+bool step_variant_ok(const phx_grid* g) {
+    return !(g->hasE && g->d.noise) && (size_t)g->d.nx * (size_t)g->d.ny < ((size_t)1 << 31);
+}
 
 // AUTO takes the fused step wherever it can run: it is 1.4-3.5x faster than the per-stage kernels on every
 // BASELINE workload; STAGE runs every model, size and term.

@@ -63,10 +63,11 @@ __device__ __forceinline__ void differences(const Coef<T>& k, const Nbhd<T>& nb,
 // K = i L - i W y + (Rr n / 2 - hgc) y - i J[other],  Kn = P - (gamr + Rr rho) n
 //   y, own:  this component's value and differences;  yo, oth: the other component's (SPINOR only)
 //   upper:   true for the psi_+ equation (operator (d_x - i d_y)^2 acts on psi_-)
-template <typename T, bool SPINOR, bool RES>
+//   Ed, q:  drive amplitude E(r) of the cell and q = (1/hbar) exp(-i omega t_s) (DRIVE only):  K += -i q E
+template <typename T, bool SPINOR, bool RES, bool DRIVE>
 __device__ __forceinline__ typename Cx<T>::type deriv(const Coef<T>& k, typename Cx<T>::type y, const Diff<T>& own,
                                                       typename Cx<T>::type yo, const Diff<T>& oth, bool upper, T nres, T V,
-                                                      T P, T& Kn) {
+                                                      T P, typename Cx<T>::type Ed, typename Cx<T>::type q, T& Kn) {
     using C = typename Cx<T>::type;
     const T rho = fma(y.y, y.y, fma(y.x, y.x, -k.doff));
     T pot = fma(k.g, rho, V);
@@ -82,7 +83,10 @@ __device__ __forceinline__ typename Cx<T>::type deriv(const Coef<T>& k, typename
         M = fma2s(-k.bxx, oth.A, M);
         M = fma2s(k.byy, oth.B, M);
     }
+    // -i q E = i (-q_re E) + q_im E: the first part joins M (rotated below), the second K
+    if (DRIVE) M = fma2s(-q.x, Ed, M);
     C K = fma2s(gain, y, rot(M));
+    if (DRIVE) K = fma2s(q.y, Ed, K);
     if (SPINOR) K = fma2s(upper ? -k.bxy : k.bxy, oth.D, K);
     Kn = RES ? P - (k.gamr + k.Rr * rho) * nres : T(0);
     return K;

@@ -28,10 +28,10 @@ template <typename T> struct StepArgs;
     cudaError_t launch_step_##P##_1(const StepArgs<T>&, bool noise, bool zbc, bool iso, int vec, dim3 grid, cudaStream_t); \
     cudaError_t launch_step_##P##_2(const StepArgs<T>&, bool noise, bool zbc, bool iso, int vec, dim3 grid, cudaStream_t); \
     cudaError_t launch_step_##P##_3(const StepArgs<T>&, bool noise, bool zbc, bool iso, int vec, dim3 grid, cudaStream_t); \
-    int occupancy_step_##P##_0(bool noise, bool zbc, bool iso, int vec);                                          \
-    int occupancy_step_##P##_1(bool noise, bool zbc, bool iso, int vec);                                          \
-    int occupancy_step_##P##_2(bool noise, bool zbc, bool iso, int vec);                                          \
-    int occupancy_step_##P##_3(bool noise, bool zbc, bool iso, int vec);
+    int occupancy_step_##P##_0(bool noise, bool zbc, bool iso, bool drive, int vec);                                          \
+    int occupancy_step_##P##_1(bool noise, bool zbc, bool iso, bool drive, int vec);                                          \
+    int occupancy_step_##P##_2(bool noise, bool zbc, bool iso, bool drive, int vec);                                          \
+    int occupancy_step_##P##_3(bool noise, bool zbc, bool iso, bool drive, int vec);
 PHX_DECL_STEP(32, float)
 PHX_DECL_STEP(64, double)
 #undef PHX_DECL_STEP

@@ -40,6 +40,7 @@ struct StepArgs {
     T* n_out[2];
     const T* V;                 // [ny][nx] or nullptr
     const T* P;                 // [ny][nx] or nullptr
+    const C* E;                 // [ny][nx] drive amplitude E(r) (kernels instantiated with DRIVE only)
     const uint64_t* step_in;    // completed steps before this one
     uint64_t* step_out;         // receives step_in + 1 (the slot the next launch reads)
     uint32_t seed;
@@ -137,7 +138,8 @@ __device__ __forceinline__ void gather(const typename Cx<T>::type (&rs)[VEC], co
 #define PHX_STEP_RING 5
 
 // MINW: resident warps per SM the register budget is sized for.  ISO: dx == dy (scalar and reservoir models only).
-template <typename T, int VEC, int MODEL, bool NOISE, bool ZBC, bool ISO, int MINW>
+// DRIVE: coherent drive E(r) exp(-i omega t) (reading Q17), shared by both components.
+template <typename T, int VEC, int MODEL, bool NOISE, bool ZBC, bool ISO, bool DRIVE, int MINW>
 __global__ void __launch_bounds__(32 * PHX_STEP_WARPS, MINW / PHX_STEP_WARPS)
 step_kernel(const __grid_constant__ StepArgs<T> a) {
     using namespace stepk;
@@ -173,6 +175,18 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
     const size_t boff = (size_t)blockIdx.z * g.plane;
     const bool zy = ZBC && g.bc_y;
 
+    // drive: q_s = (1/hbar) exp(-i omega t_s) at the stage times t, t + dt/2, t + dt, t = step dt; the phase is evaluated
+    // in double and rounded to T (reading Q17)
+    C q1 = mk<T>(T(0), T(0)), q23 = q1, q4 = q1;
+    if constexpr (DRIVE) {
+        auto phase = [&](double cs) {
+            double sn, cn;
+            sincos(-k.omega * (((double)step + cs) * k.dt_d), &sn, &cn);
+            return mk<T>(k.ih * (T)cn, k.ih * (T)sn);
+        };
+        q1 = phase(0.0); q23 = phase(0.5); q4 = phase(1.0);
+    }
+
     // ---- base pointers of this realisation (warp-uniform); rows and columns are addressed by 32-bit cell offsets ----
     const C* pin[NC];
     C* pout[NC];
@@ -187,13 +201,14 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
     }
     const T* Vp = a.V;
     const T* Pp = RES ? a.P : nullptr;
+    const C* Ep = DRIVE ? a.E : nullptr;
     // keep the bases as they are: one 64-bit register pair each, every access = base + (32-bit cell offset) * size
 #pragma unroll
     for (int s = 0; s < NC; ++s) {
         asm volatile("" : "+l"(pin[s]), "+l"(pout[s]));
         if (RES) asm volatile("" : "+l"(nin[s]), "+l"(nout_p[s]));
     }
-    asm volatile("" : "+l"(Vp), "+l"(Pp));
+    asm volatile("" : "+l"(Vp), "+l"(Pp), "+l"(Ep));
 
     // ---- register rings (slot of row q = q mod RING; see the note above) ---------------------------------------------
     const C czero = mk<T>(T(0), T(0));
@@ -203,6 +218,7 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
     C y4r[NC][RING][VEC];                   // stage-4 input: rows j-4, j-3 carried, row j-2 produced
     C accr[NC][RING][VEC];                  // running sum of Eq. (6): row j produced, rows j-1 .. j-3 updated / consumed
     T Vr[RING][VEC], Pr[RING][VEC];         // V, P: rows j-3 .. j live, row j+1 in flight
+    C Er[RING][VEC];                        // drive amplitude, as V
     T nr[NC][RING][VEC];                    // reservoir n(t): rows j-3 .. j live, row j+1 in flight
     T n2r[NC][RING][VEC], n3r[NC][RING][VEC], n4r[NC][RING][VEC];   // reservoir stage inputs (cell-local)
     T naccr[NC][RING][VEC];                 // reservoir running sum
@@ -215,7 +231,7 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
                 psr[s][r][i] = czero; y2r[s][r][i] = czero; y3r[s][r][i] = czero; y4r[s][r][i] = czero; accr[s][r][i] = czero;
                 nr[s][r][i] = T(0); n2r[s][r][i] = T(0); n3r[s][r][i] = T(0); n4r[s][r][i] = T(0); naccr[s][r][i] = T(0);
             }
-            Vr[r][i] = T(0); Pr[r][i] = T(0);
+            Vr[r][i] = T(0); Pr[r][i] = T(0); Er[r][i] = czero;
         }
     }
 
@@ -246,6 +262,7 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
                 }
                 if (Vp) prefetch_l2(Vp + e);
                 if (Pp) prefetch_l2(Pp + e);
+                if (DRIVE) prefetch_l2(Ep + e);
             }
             ++q; e += nx;
             if (!zy && q == ny) { q = 0; e -= plane; }
@@ -264,6 +281,7 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
         if (d == 0 && okq) {
             if (Vp) ldr<VEC>(Vp + ew, Vr[(d + R2) % RING]);
             if (Pp) ldr<VEC>(Pp + ew, Pr[(d + R2) % RING]);
+            if (DRIVE) ldc<VEC>(Ep + ew, Er[(d + R2) % RING]);
             if constexpr (RES) {
 #pragma unroll
                 for (int s = 0; s < NC; ++s) ldr<VEC>(nin[s] + ew, nr[s][(d + R2) % RING]);
@@ -294,6 +312,7 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
                     }
                     if (Vp) prefetch_l2(Vp + e);
                     if (Pp) prefetch_l2(Pp + e);
+                    if (DRIVE) prefetch_l2(Ep + e);
                 } else if (inx && (j + 2 + pfr <= r1 + 3) && qw + pfr < ny && qw + pfr >= 0) {
 #pragma unroll
                     for (int s = 0; s < NC; ++s) {
@@ -302,6 +321,7 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
                     }
                     if (Vp) prefetch_l2(Vp + ew + epf);
                     if (Pp) prefetch_l2(Pp + ew + epf);
+                    if (DRIVE) prefetch_l2(Ep + ew + epf);
                 }
             }
             // ---- fetch: psi row j+2; row-local inputs (V, P, n) of row j+1 -------------------------------------------------
@@ -318,11 +338,12 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
             }
             if (ZBC) {              // (periodic without V or P: the slots keep the zeros they were initialised with)
 #pragma unroll
-                for (int i = 0; i < VEC; ++i) { Vr[SL(1)][i] = T(0); Pr[SL(1)][i] = T(0); }
+                for (int i = 0; i < VEC; ++i) { Vr[SL(1)][i] = T(0); Pr[SL(1)][i] = T(0); Er[SL(1)][i] = czero; }
             }
             if (okprev) {
                 if (Vp) ldr<VEC>(Vp + ewp, Vr[SL(1)]);
                 if (Pp) ldr<VEC>(Pp + ewp, Pr[SL(1)]);
+                if (DRIVE) ldc<VEC>(Ep + ewp, Er[SL(1)]);
             }
             if constexpr (RES) {
 #pragma unroll
@@ -361,7 +382,7 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
                     for (int i = 0; i < VEC; ++i) {
                         T Kn;
                         const T nres = RES ? nr[s][SL(0)][i] : T(0);
-                        const C K = deriv<T, SPINOR, RES>(k, nb[s][i].c, df[s][i], nb[O(s)][i].c, df[O(s)][i], s == 0, nres, Vr[SL(0)][i], Pr[SL(0)][i], Kn);
+                        const C K = deriv<T, SPINOR, RES, DRIVE>(k, nb[s][i].c, df[s][i], nb[O(s)][i].c, df[O(s)][i], s == 0, nres, Vr[SL(0)][i], Pr[SL(0)][i], Er[SL(0)][i], q1, Kn);
                         const C p = psr[s][SL(0)][i];
                         y2r[s][SL(0)][i] = in1 ? fma2s(k.hdt, K, p) : czero;
                         accr[s][SL(0)][i] = fma2s(k.dt6, K, p);
@@ -379,7 +400,7 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
                     for (int i = 0; i < VEC; ++i) {
                         T Kn;
                         const T nres = RES ? n2r[s][SL(-1)][i] : T(0);
-                        const C K = deriv<T, SPINOR, RES>(k, nb[s][i].c, df[s][i], nb[O(s)][i].c, df[O(s)][i], s == 0, nres, Vr[SL(-1)][i], Pr[SL(-1)][i], Kn);
+                        const C K = deriv<T, SPINOR, RES, DRIVE>(k, nb[s][i].c, df[s][i], nb[O(s)][i].c, df[O(s)][i], s == 0, nres, Vr[SL(-1)][i], Pr[SL(-1)][i], Er[SL(-1)][i], q23, Kn);
                         const C p = psr[s][SL(-1)][i];
                         y3r[s][SL(-1)][i] = in2 ? fma2s(k.hdt, K, p) : czero;
                         accr[s][SL(-1)][i] = fma2s(k.dt3, K, accr[s][SL(-1)][i]);
@@ -397,7 +418,7 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
                     for (int i = 0; i < VEC; ++i) {
                         T Kn;
                         const T nres = RES ? n3r[s][SL(-2)][i] : T(0);
-                        const C K = deriv<T, SPINOR, RES>(k, nb[s][i].c, df[s][i], nb[O(s)][i].c, df[O(s)][i], s == 0, nres, Vr[SL(-2)][i], Pr[SL(-2)][i], Kn);
+                        const C K = deriv<T, SPINOR, RES, DRIVE>(k, nb[s][i].c, df[s][i], nb[O(s)][i].c, df[O(s)][i], s == 0, nres, Vr[SL(-2)][i], Pr[SL(-2)][i], Er[SL(-2)][i], q23, Kn);
                         const C p = psr[s][SL(-2)][i];
                         y4r[s][SL(-2)][i] = in3 ? fma2s(k.dt, K, p) : czero;
                         accr[s][SL(-2)][i] = fma2s(k.dt3, K, accr[s][SL(-2)][i]);
@@ -419,7 +440,7 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
                     for (int i = 0; i < VEC; ++i) {
                         T Kn;
                         const T nres = RES ? n4r[s][SL(-3)][i] : T(0);
-                        const C K = deriv<T, SPINOR, RES>(k, nb[s][i].c, df[s][i], nb[O(s)][i].c, df[O(s)][i], s == 0, nres, Vr[SL(-3)][i], Pr[SL(-3)][i], Kn);
+                        const C K = deriv<T, SPINOR, RES, DRIVE>(k, nb[s][i].c, df[s][i], nb[O(s)][i].c, df[O(s)][i], s == 0, nres, Vr[SL(-3)][i], Pr[SL(-3)][i], Er[SL(-3)][i], q4, Kn);
                         out[i] = fma2s(k.dt6, K, accr[s][SL(-3)][i]);
                         nout[i] = RES ? naccr[s][SL(-3)][i] + k.dt6 * Kn : T(0);
                     }

@@ -37,17 +37,17 @@ typedef double real_t;
 #define PHX_HAS_VEC4 (PHX_INST_PREC == 32 && PHX_INST_MODEL == 0)
 #endif
 
-template <int VEC, bool NOISE, bool ZBC, bool ISO>
+template <int VEC, bool NOISE, bool ZBC, bool ISO, bool DRIVE>
 struct Inst {
     static constexpr int MINW = VEC == 4 ? 8 : (VEC == 2 ? PHX_MINW_V2 : PHX_MINW_V1);
     static constexpr bool I = ISO && PHX_HAS_ISO;
     static cudaError_t launch(const StepArgs<real_t>& a, dim3 grid, cudaStream_t st) {
-        step_kernel<real_t, VEC, PHX_INST_MODEL, NOISE, ZBC, I, MINW><<<grid, 32 * PHX_STEP_WARPS, 0, st>>>(a);
+        step_kernel<real_t, VEC, PHX_INST_MODEL, NOISE, ZBC, I, DRIVE, MINW><<<grid, 32 * PHX_STEP_WARPS, 0, st>>>(a);
         return cudaGetLastError();
     }
     static int occupancy() {   // resident CTAs per SM
         int nb = 0;
-        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, step_kernel<real_t, VEC, PHX_INST_MODEL, NOISE, ZBC, I, MINW>,
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, step_kernel<real_t, VEC, PHX_INST_MODEL, NOISE, ZBC, I, DRIVE, MINW>,
                                                           32 * PHX_STEP_WARPS, 0) != cudaSuccess) {
             cudaGetLastError();
             return MINW / PHX_STEP_WARPS;
@@ -56,24 +56,28 @@ struct Inst {
     }
 };
 
+// The driven kernels are instantiated without noise (a driven noisy grid runs variant STAGE).
+template <int VEC, bool NOISE, bool DRIVE, typename F>
+static auto dispatch2(bool zbc, bool iso, F f) {
+    if (zbc) return iso ? f(Inst<VEC, NOISE, true, true, DRIVE>()) : f(Inst<VEC, NOISE, true, false, DRIVE>());
+    return iso ? f(Inst<VEC, NOISE, false, true, DRIVE>()) : f(Inst<VEC, NOISE, false, false, DRIVE>());
+}
+
 template <int VEC, typename F>
-static auto dispatch(bool noise, bool zbc, bool iso, F f) {
-    if (noise) {
-        if (zbc) return iso ? f(Inst<VEC, true, true, true>()) : f(Inst<VEC, true, true, false>());
-        return iso ? f(Inst<VEC, true, false, true>()) : f(Inst<VEC, true, false, false>());
-    }
-    if (zbc) return iso ? f(Inst<VEC, false, true, true>()) : f(Inst<VEC, false, true, false>());
-    return iso ? f(Inst<VEC, false, false, true>()) : f(Inst<VEC, false, false, false>());
+static auto dispatch(bool noise, bool zbc, bool iso, bool drive, F f) {
+    if (noise) return dispatch2<VEC, true, false>(zbc, iso, f);
+    if (drive) return dispatch2<VEC, false, true>(zbc, iso, f);
+    return dispatch2<VEC, false, false>(zbc, iso, f);
 }
 
 template <int VEC>
-static int occ_vec(bool noise, bool zbc, bool iso) {
-    return dispatch<VEC>(noise, zbc, iso, [](auto inst) { return decltype(inst)::occupancy(); });
+static int occ_vec(bool noise, bool zbc, bool iso, bool drive) {
+    return dispatch<VEC>(noise, zbc, iso, drive, [](auto inst) { return decltype(inst)::occupancy(); });
 }
 
 template <int VEC>
 static cudaError_t launch_vec(const StepArgs<real_t>& a, bool noise, bool zbc, bool iso, dim3 grid, cudaStream_t st) {
-    return dispatch<VEC>(noise, zbc, iso, [&](auto inst) { return decltype(inst)::launch(a, grid, st); });
+    return dispatch<VEC>(noise, zbc, iso, a.E != nullptr, [&](auto inst) { return decltype(inst)::launch(a, grid, st); });
 }
 
 #define PHX_CAT3(a, b, c) a##b##_##c
@@ -96,16 +100,16 @@ cudaError_t PHX_NAME(PHX_INST_PREC, PHX_INST_MODEL)(const StepArgs<real_t>& a, b
 #define PHX_OCC_NAME(p, m) PHX_CAT3(occupancy_step_, p, m)
 
 // Resident CTAs per SM of the instantiation (for the launch plan: one balanced wave).
-int PHX_OCC_NAME(PHX_INST_PREC, PHX_INST_MODEL)(bool noise, bool zbc, bool iso, int vec) {
+int PHX_OCC_NAME(PHX_INST_PREC, PHX_INST_MODEL)(bool noise, bool zbc, bool iso, bool drive, int vec) {
 #if PHX_INST_PREC == 32
 #if PHX_HAS_VEC4
-    if (vec == 4) return occ_vec<4>(noise, zbc, iso);
+    if (vec == 4) return occ_vec<4>(noise, zbc, iso, drive);
 #endif
-    if (vec == 2) return occ_vec<2>(noise, zbc, iso);
+    if (vec == 2) return occ_vec<2>(noise, zbc, iso, drive);
 #elif PHX_HAS_VEC2_64
-    if (vec == 2) return occ_vec<2>(noise, zbc, iso);
+    if (vec == 2) return occ_vec<2>(noise, zbc, iso, drive);
 #endif
-    return occ_vec<1>(noise, zbc, iso);
+    return occ_vec<1>(noise, zbc, iso, drive);
 }
 
 }  // namespace phx

@@ -120,24 +120,54 @@ def test_density_offset():
     run_pair(w, 50, extra_params=dict(density_offset=0.02))
 
 
-def test_drive_is_not_available_in_the_fused_step():
+def _drive_field(w, seed=30):
+    rng = np.random.default_rng(seed)
+    return (0.05 * (rng.standard_normal((w.ny, w.nx)) + 1j * rng.standard_normal((w.ny, w.nx)))).astype(
+        np.complex64 if w.prec == "c32" else np.complex128)
+
+
+@pytest.mark.parametrize("prec", ["c32", "c64"])
+@pytest.mark.parametrize("model", ["scalar", "reservoir", "spinor", "spinor_reservoir"])
+def test_coherent_drive(prec, model):
+    # E(r) exp(-i omega t) at the stage times t, t + dt/2, t + dt (reading Q17)
+    w = {"scalar": lambda: wl.cfg2(n=140, ny=90, prec=prec), "reservoir": lambda: wl.cfg3(n=96, prec=prec),
+         "spinor": lambda: wl.cfg4(n=96, prec=prec, sigma_cells=10.0), "spinor_reservoir": lambda: wl.example3(n=90, prec=prec)}[model]()
+    run_pair(w, 101, E=_drive_field(w), extra_params=dict(omega=3.7))
+
+
+@pytest.mark.parametrize("tuning,bc", [({"step_vec": 4}, (0, 0)), ({"step_vec": 2, "step_ly": 9}, (1, 1)), ({"step_vec": 1}, (0, 1))])
+def test_coherent_drive_cells_per_lane_and_boundaries(tuning, bc):
+    w = wl.cfg2(n=132, ny=70, prec="c32")
+    w = dataclasses.replace(w, dy=w.dx * 1.1)
+    run_pair(w, 60, E=_drive_field(w), extra_params=dict(omega=-2.1), tuning=tuning, bc=bc)
+
+
+def test_drive_set_mid_run_and_driven_noise_falls_back_to_stage():
     from paper_2411_18341_b200 import binding as phx
     w = wl.cfg2(n=64, ny=32, prec="c32")
-    E = np.zeros((w.ny, w.nx), np.complex64)
-    g = make_gpu(w, E=E)
-    with pytest.raises(phx.PhxError) as e:
-        g.select_variant(STEP)
-    assert e.value.status == phx.PHX_ERR_UNSUPPORTED
-    g.destroy()
-    g = make_gpu(w, variant=STEP)
+    E = _drive_field(w)
+    xp = dict(omega=1.3)
+    g = make_gpu(w, variant=STEP, extra_params=xp)
     g.step_rk4(3)                                  # odd: state in the alternate buffer
-    g.set_drive(E)                                 # falls back to STAGE and moves the state back
-    assert g.get_variant() == STAGE
+    g.set_drive(E)                                 # the fused step carries on, now with the drive
+    assert g.get_variant() == STEP
     g.step_rk4(2)
-    o = make_oracle(w, E=E)
-    o.step_rk4(5)
-    compare(g, o, w)
+    o = make_oracle(w, extra_params=xp)
+    o.step_rk4(3)
+    o2 = make_oracle(w, E=E, extra_params=xp)
+    o2.set_field("psi_p", o.psi_p)
+    o2.step = 3
+    o2.step_rk4(2)
+    assert rel_l2(g.read_field("psi_p"), o2.psi_p) <= TOL["c32"]
     g.destroy()
+    # a driven grid with noise: the driven fused kernels are built without noise, AUTO takes the per-stage kernels
+    wn = wl.cfg5(n=64, batch=2)
+    gn = make_gpu(wn, E=_drive_field(wn))
+    assert gn.get_variant() == STAGE
+    with pytest.raises(phx.PhxError) as e:
+        gn.select_variant(STEP)
+    assert e.value.status == phx.PHX_ERR_UNSUPPORTED
+    gn.destroy()
 
 
 # ---- stochastic path -------------------------------------------------------------------------------------

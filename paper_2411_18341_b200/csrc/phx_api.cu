@@ -90,6 +90,7 @@ struct phx_grid {
     cudaGraphExec_t g1[2], gN;  // one step from parity 0 / 1; graph_steps steps from parity 0
     bool graphs_valid;
     int n_sm;
+    size_t l2_bytes;        // L2 capacity of the device
     cudaError_t sticky;
     std::string err;
 };
@@ -263,22 +264,47 @@ int step_occupancy(const phx_grid* g, int vec) {
     }
 }
 
-// Rows per chunk: every CTA costs (ly + 9) row iterations (4 + 4 halo rows and the pipeline fill) rounded up to the
-// unroll factor of the row loop (5, the ring length), and the grid runs in ceil(CTAs / resident CTAs) waves; pick the
-// chunk count that minimises waves * iterations.
+// Bytes one step of variant STEP touches per cell (state in and out, V, P, E).
+size_t step_bytes_per_cell(const phx_grid* g) {
+    const size_t rb = real_bytes(g);
+    const size_t nc = model_spinor(g->d.model) ? 2 : 1;
+    size_t b = nc * 4 * rb;
+    if (model_reservoir(g->d.model)) b += nc * 2 * rb;
+    if (g->hasV) b += rb;
+    if (g->hasP) b += rb;
+    if (g->hasE) b += 2 * rb;
+    return b;
+}
+
+// Rows per chunk.  Every CTA costs (ly + 6) row iterations (4 + 4 halo rows and the pipeline fill, less the two rows
+// the prologue fetches) rounded up to the unroll factor of the row loop (5, the ring length).
+//  - Working set beyond L2 (the BASELINE grids from 4096^2 up, cfg5): an iteration waits on DRAM, more resident warps
+//    hide it, and the grid runs in ceil(CTAs / resident CTAs) waves: minimise waves * iterations.
+//  - Working set within half of L2 (1024^2): two warps per scheduler already saturate the FP32 pipe (measured at
+//    1024^2 fp32: 525 cycles per iteration with 1-2 warps per scheduler, 810 with 3, 1250 with 4), so fewer, longer
+//    chunks win: minimise iterations * max(1.75, warps per scheduler) (ly = 19 instead of 9: 113 instead of 80
+//    Gcell*step/s).
 int step_rows_per_chunk(const phx_grid* g, int vec) {
     if (g->step_ly) return g->step_ly < g->d.ny ? g->step_ly : g->d.ny;
     const int strips = (g->d.nx + 32 * vec - 9) / (32 * vec - 8);
     const long ctas_row = (long)((strips + PHX_STEP_WARPS - 1) / PHX_STEP_WARPS) * g->d.batch;
     const long slots = (long)g->n_sm * step_occupancy(g, vec);
-    long best_cost = -1;
+    const bool in_l2 = plane_cells(g) * g->d.batch * step_bytes_per_cell(g) < g->l2_bytes / 2;
+    double best_cost = -1;
     int best_ly = g->d.ny;
     const int max_chunks = g->d.ny / 8 > 0 ? g->d.ny / 8 : 1;
     for (int nch = 1; nch <= max_chunks && nch <= 65535; ++nch) {
         const int ly = (g->d.ny + nch - 1) / nch;
         const int real_chunks = (g->d.ny + ly - 1) / ly;
-        const long waves = (ctas_row * real_chunks + slots - 1) / slots;
-        const long cost = waves * ((ly + 9 + 4) / 5 * 5);
+        const long ctas = ctas_row * real_chunks;
+        const long waves = (ctas + slots - 1) / slots;
+        const long iters = (ly + 6 + 4) / 5 * 5;
+        double cost = (double)(waves * iters);
+        if (in_l2) {
+            const long per_sm = ((ctas + waves - 1) / waves + g->n_sm - 1) / g->n_sm;     // CTAs on the fullest SM
+            const long per_sched = (per_sm * PHX_STEP_WARPS + 3) / 4;
+            cost *= per_sched > 1.75 ? (double)per_sched : 1.75;
+        }
         if (best_cost < 0 || cost < best_cost) { best_cost = cost; best_ly = ly; }
     }
     return best_ly;
@@ -466,6 +492,7 @@ phx_status phx_create_grid(phx_grid** out, const phx_grid_desc* desc) {
     g->parity = 0;
     g->step_ly = g->step_vec = 0;
     g->n_sm = prop.multiProcessorCount;
+    g->l2_bytes = (size_t)prop.l2CacheSize;
     g->sticky = cudaSuccess;
     g->variant = PHX_VARIANT_STAGE;
     resolve_variant(g);

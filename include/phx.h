@@ -65,7 +65,6 @@ typedef enum {
     PHX_VARIANT_STAGE = 1,     /* one fused kernel per RK stage (4 launches per step); every model and term */
     PHX_VARIANT_STEP = 3,      /* one kernel per RK4 step: the four stages pipelined along y in register windows of
                                   a haloed warp-wide column strip (N_halo = 4); not for drive + noise together */
-    PHX_VARIANT_RESIDENT = 4   /* whole grid resident on chip, many steps per launch (small grids) */
 } phx_variant;
 
 typedef struct {

@@ -19,7 +19,7 @@ PHX_SCALAR, PHX_RESERVOIR, PHX_SPINOR, PHX_SPINOR_RESERVOIR = range(4)
 PHX_HOST, PHX_DEVICE = 0, 1
 PHX_PSI, PHX_PSI_MINUS, PHX_N, PHX_N_MINUS = range(4)
 PHX_BC_PERIODIC, PHX_BC_ZERO = 0, 1
-PHX_VARIANT_AUTO, PHX_VARIANT_STAGE, PHX_VARIANT_STEP = 0, 1, 3
+PHX_VARIANT_AUTO, PHX_VARIANT_STAGE, PHX_VARIANT_STEP, PHX_VARIANT_RESIDENT = 0, 1, 3, 4
 PHX_NCOEF = 18
 
 MODELS = {"scalar": PHX_SCALAR, "reservoir": PHX_RESERVOIR, "spinor": PHX_SPINOR, "spinor_reservoir": PHX_SPINOR_RESERVOIR}

@@ -361,7 +361,27 @@ cudaError_t enqueue_step_fused(phx_grid* g, cudaStream_t st, int parity) {
     }
 }
 
-int kernels_per_step(const phx_grid* g) { return g->variant == PHX_VARIANT_STEP ? 1 : 4; }
+int kernels_per_step(const phx_grid* g) { return g->variant == PHX_VARIANT_STEP ? 1 : 4; }   // (RESIDENT: one per call)
+
+// Variant RESIDENT: all n steps in one launch, in place on the buffers of the current parity.
+template <typename T>
+cudaError_t launch_resident(phx_grid* g, int n_steps) {
+    using C = typename Cx<T>::type;
+    ResidentArgs<T> a;
+    std::memset(&a, 0, sizeof(a));
+    fill_geo_coef<T>(g, a.geo, a.k);
+    const bool res = model_reservoir(g->d.model);
+    a.psi = (C*)(g->ws + (g->parity ? g->L.ya[0] : g->L.psi[0]));
+    a.n = res ? (T*)(g->ws + (g->parity ? g->L.na[0] : g->L.n[0])) : nullptr;
+    a.V = g->hasV ? (const T*)(g->ws + g->L.V) : nullptr;
+    a.P = g->hasP ? (const T*)(g->ws + g->L.P) : nullptr;
+    a.step_slots = (uint64_t*)(g->ws + g->L.step);
+    a.step0 = g->step_host;
+    a.n_steps = n_steps;
+    a.seed = g->prm.seed;
+    if constexpr (sizeof(T) == 4) return launch_resident_32(a, res, g->d.noise != 0, g->stream);
+    else return launch_resident_64(a, res, g->d.noise != 0, g->stream);
+}
 
 // Enqueues one step starting from state parity `parity` (always 0 for variant STAGE).
 cudaError_t enqueue_step(phx_grid* g, cudaStream_t st, int parity) {
@@ -392,10 +412,21 @@ bool step_variant_ok(const phx_grid* g) {
     return !(g->hasE && g->d.noise) && (size_t)g->d.nx * (size_t)g->d.ny < ((size_t)1 << 31);
 }
 
-// AUTO takes the fused step wherever it can run: it is 1.4-3.5x faster than the per-stage kernels on every
-// BASELINE workload; STAGE runs every model, size and term.
+// Variant RESIDENT: scalar and reservoir models without drive whose grid fits one CTA (phx_resident.cu).
+bool resident_variant_ok(const phx_grid* g) {
+    if (model_spinor(g->d.model) || g->hasE) return false;
+    return resident_cpt(g->d.nx * g->d.ny, g->d.prec == PHX_C64, model_reservoir(g->d.model)) != 0;
+}
+
+// AUTO takes the resident kernel for ensembles of grids that fit it (one CTA per realisation: 2.3x the fused step on
+// 512 x 64^2 fp32; a single small grid is faster spread over several SMs by the fused step: 3.9 against 4.3 us per step at
+// 64^2 fp32), else the fused step wherever it can run (1.4-4.7x faster than the per-stage kernels on every BASELINE
+// workload); STAGE runs every model, size and term.
 void resolve_variant(phx_grid* g) {
-    if (g->variant_req != PHX_VARIANT_STAGE && step_variant_ok(g)) g->variant = PHX_VARIANT_STEP;
+    const int req = g->variant_req;
+    const bool res_ok = resident_variant_ok(g);
+    if (res_ok && (req == PHX_VARIANT_RESIDENT || (req == PHX_VARIANT_AUTO && g->d.batch >= 32))) g->variant = PHX_VARIANT_RESIDENT;
+    else if (req != PHX_VARIANT_STAGE && step_variant_ok(g)) g->variant = PHX_VARIANT_STEP;
     else g->variant = PHX_VARIANT_STAGE;
 }
 
@@ -422,7 +453,7 @@ phx_status apply_variant(phx_grid* g) {
     const int before = g->variant;
     resolve_variant(g);
     drop_graphs(g);
-    if (before == PHX_VARIANT_STEP && g->variant != PHX_VARIANT_STEP) return normalise_state(g);
+    if (g->variant == PHX_VARIANT_STAGE) return normalise_state(g);   // STAGE keeps the state in psi/n
     return PHX_OK;
 }
 
@@ -589,6 +620,16 @@ phx_status phx_step_rk4(phx_grid* g, int64_t n_steps) {
     if (g->sticky != cudaSuccess) return PHX_ERR_CUDA;
     if (!g->has_params) return fail(g, PHX_ERR_BAD_STATE, "phx_step_rk4: call phx_set_params first");
     if (n_steps == 0) return PHX_OK;
+    if (g->variant == PHX_VARIANT_RESIDENT) {
+        for (int64_t left = n_steps; left > 0;) {
+            const int chunk = left > (1 << 30) ? (1 << 30) : (int)left;
+            PHX_CUDA(g, g->d.prec == PHX_C64 ? launch_resident<double>(g, chunk) : launch_resident<float>(g, chunk));
+            g->step_host += (uint64_t)chunk;
+            g->launches += 1;
+            left -= chunk;
+        }
+        return PHX_OK;
+    }
     if (!g->graphs_valid) {
         drop_graphs(g);
         PHX_CUDA(g, capture(g, 1, 0, &g->g1[0]));
@@ -682,7 +723,8 @@ phx_status phx_debug_noise_u32(phx_grid* g, uint64_t step, uint32_t* dst, phx_me
 phx_status phx_select_variant(phx_grid* g, int32_t variant) {
     if (!g) return PHX_ERR_INVALID_ARG;
     if (g->sticky != cudaSuccess) return PHX_ERR_CUDA;
-    if (variant != PHX_VARIANT_AUTO && variant != PHX_VARIANT_STAGE && !(variant == PHX_VARIANT_STEP && step_variant_ok(g)))
+    if (variant != PHX_VARIANT_AUTO && variant != PHX_VARIANT_STAGE && !(variant == PHX_VARIANT_STEP && step_variant_ok(g)) &&
+        !(variant == PHX_VARIANT_RESIDENT && resident_variant_ok(g)))
         return fail(g, PHX_ERR_UNSUPPORTED, "phx_select_variant: variant not available for this grid/model");
     g->variant_req = variant;
     return apply_variant(g);

@@ -36,6 +36,27 @@ PHX_DECL_STEP(32, float)
 PHX_DECL_STEP(64, double)
 #undef PHX_DECL_STEP
 
+// phx_resident.cu: variant RESIDENT (a small grid on chip for all steps of one launch)
+#ifndef PHX_RESIDENT_THREADS
+#define PHX_RESIDENT_THREADS 512
+#endif
+template <typename T>
+struct ResidentArgs {
+    Geom geo;
+    Coef<T> k;
+    typename Cx<T>::type* psi;      // state [batch][ny][nx], advanced in place
+    T* n;                           // reservoir state, or nullptr
+    const T* V;                     // [ny][nx] or nullptr
+    const T* P;                     // [ny][nx] or nullptr
+    uint64_t* step_slots;           // both device step-counter slots receive step0 + n_steps
+    uint64_t step0;                 // completed steps before this launch
+    int n_steps;
+    uint32_t seed;
+};
+int resident_cpt(int cells, int prec64, bool res);     // cells per thread, 0 = the grid does not fit
+cudaError_t launch_resident_32(const ResidentArgs<float>&, bool res, bool noise, cudaStream_t);
+cudaError_t launch_resident_64(const ResidentArgs<double>&, bool res, bool noise, cudaStream_t);
+
 // phx_aux.cu: small helper kernels
 cudaError_t launch_ensemble_mean(const void* psi, void* out, int prec64, size_t plane, int batch, cudaStream_t);
 cudaError_t launch_noise_words(uint32_t* out, uint32_t seed, uint64_t step, size_t plane, int r0, int batch, cudaStream_t);

@@ -1,0 +1,181 @@
+// phx_resident.cu -- variant RESIDENT: a small grid stays on chip for many RK4 steps of one launch
+// (SURVEY.md section 8(a) "V-small persistent"; the paper's small-grid regime is bound by kernel-launch latency,
+// PAPER.md:289, which CUDA graphs only soften, :195).
+//
+// One CTA of 512 threads owns one realisation (blockIdx.x).  A thread owns CPT cells (cell c = tid + k*512) and keeps
+// their psi(t), the running sum of Eq. (6) and the reservoir values in registers for the whole launch.  The stage
+// input y_s, of which a cell needs its four neighbours (Eq. (8)), lives in two shared-memory buffers that alternate:
+// stage s reads buffer A and writes y_{s+1} into buffer B, one __syncthreads per stage, four per step (Eqs. (2)-(6),
+// PAPER.md:53-62).  V, P and the four neighbour indices of every cell (periodic wrap, or a zero cell beyond a zero
+// boundary) are staged in shared memory once.  HBM traffic: the state in at the first step and out at the
+// last.  Scalar and reservoir models, both precisions, optional noise (Eq. (22)); no drive.
+// The derivative is the one of variant STEP (phx_deriv.cuh).  Product code: shares nothing with oracle/.
+#include "phx_common.cuh"
+#include "phx_deriv.cuh"
+#include "phx_philox.cuh"
+#include "phx_launch.h"
+
+#include <type_traits>
+
+namespace phx {
+
+constexpr int RES_NT = PHX_RESIDENT_THREADS;
+
+template <typename T, bool RES, bool NOISE, int CPT>
+__global__ void __launch_bounds__(RES_NT, 1)
+resident_kernel(const __grid_constant__ ResidentArgs<T> a) {
+    using C = typename Cx<T>::type;
+    extern __shared__ __align__(16) unsigned char smem[];
+    const Geom& g = a.geo;
+    const Coef<T>& k = a.k;
+    const int nx = g.nx, ny = g.ny, N = nx * ny;
+    // shared memory: two stage buffers of N + 1 complex (cell N holds 0), neighbour indices, V, P
+    C* buf0 = reinterpret_cast<C*>(smem);
+    C* buf1 = buf0 + (N + 1);
+    ushort4* nbr = reinterpret_cast<ushort4*>(buf1 + (N + 1));      // w, e, s (row j-1), n (row j+1)
+    T* Vs = reinterpret_cast<T*>(nbr + N);
+    T* Ps = Vs + N;
+
+    const int tid = threadIdx.x;
+    const size_t boff = (size_t)blockIdx.x * g.plane;
+    C* psi_g = a.psi + boff;
+    T* n_g = RES ? a.n + boff : nullptr;
+    const C czero = mk<T>(T(0), T(0));
+
+    C psi[CPT], acc[CPT];
+    T nn[CPT], nacc[CPT], nst[CPT];
+#pragma unroll
+    for (int q = 0; q < CPT; ++q) {
+        const int c = tid + q * RES_NT;
+        psi[q] = czero; acc[q] = czero; nn[q] = T(0); nacc[q] = T(0); nst[q] = T(0);
+        if (c < N) {
+            const int j = c / nx, i = c - j * nx;
+            ushort4 nb;
+            nb.x = (unsigned short)(i > 0 ? c - 1 : (g.bc_x ? N : c + nx - 1));
+            nb.y = (unsigned short)(i < nx - 1 ? c + 1 : (g.bc_x ? N : c - nx + 1));
+            nb.z = (unsigned short)(j > 0 ? c - nx : (g.bc_y ? N : c + N - nx));
+            nb.w = (unsigned short)(j < ny - 1 ? c + nx : (g.bc_y ? N : c - N + nx));
+            nbr[c] = nb;
+            Vs[c] = a.V ? a.V[c] : T(0);
+            Ps[c] = (RES && a.P) ? a.P[c] : T(0);
+            psi[q] = psi_g[c];
+            if (RES) nn[q] = n_g[c];
+            buf0[c] = psi[q];
+        }
+    }
+    if (tid == 0) { buf0[N] = czero; buf1[N] = czero; }
+    __syncthreads();
+
+    // one stage: K_s from the stage input in `in`; a_dt = a_s dt of Eqs. (3)-(5), w_dt = weight of K_s in Eq. (6)
+    auto stage = [&](const C* in, C* out, auto stage_no, const uint64_t step) {
+        constexpr int s = decltype(stage_no)::value;
+        const T a_dt = s == 3 ? k.dt : k.hdt;
+        const T w_dt = (s == 1 || s == 4) ? k.dt6 : k.dt3;
+#pragma unroll
+        for (int q = 0; q < CPT; ++q) {
+            const int c = tid + q * RES_NT;
+            if (c < N) {
+                const ushort4 nb = nbr[c];
+                Nbhd<T> h;
+                h.c = s == 1 ? psi[q] : in[c];
+                h.w = in[nb.x]; h.e = in[nb.y]; h.s = in[nb.z]; h.n = in[nb.w];
+                Diff<T> df;
+                differences<T, false, false>(k, h, df);
+                const T nres = RES ? (s == 1 ? nn[q] : nst[q]) : T(0);
+                T Kn;
+                const C K = deriv<T, false, RES, false>(k, h.c, df, czero, df, true, nres, Vs[c], Ps[c], czero, czero, Kn);
+                if (s == 1) {
+                    acc[q] = fma2s(w_dt, K, psi[q]);
+                    if (RES) nacc[q] = nn[q] + w_dt * Kn;
+                } else if (s < 4) {
+                    acc[q] = fma2s(w_dt, K, acc[q]);
+                    if (RES) nacc[q] += w_dt * Kn;
+                }
+                if (s < 4) {
+                    out[c] = fma2s(a_dt, K, psi[q]);
+                    if (RES) nst[q] = nn[q] + a_dt * Kn;
+                } else {
+                    C nw = fma2s(w_dt, K, acc[q]);
+                    if (NOISE) {
+                        const uint4 wd = noise_words(a.seed, blockIdx.x, step, (uint32_t)c);
+                        const C xi = normal_pair(wd.x, wd.y, T(0));
+                        const T nt = RES ? nn[q] : T(0);          // reservoir at the start of the step
+                        const T sigma = sqrt(k.sig2 * (T(2) * k.hgc + k.Rr * nt));
+                        nw = fma2s(sigma, xi, nw);
+                    }
+                    psi[q] = nw;
+                    if (RES) nn[q] = nacc[q] + w_dt * Kn;
+                    out[c] = nw;                                  // stage-1 input of the next step
+                }
+            }
+        }
+        __syncthreads();
+    };
+
+    for (int it = 0; it < a.n_steps; ++it) {
+        const uint64_t step = a.step0 + (uint64_t)it;
+        stage(buf0, buf1, std::integral_constant<int, 1>(), step);
+        stage(buf1, buf0, std::integral_constant<int, 2>(), step);
+        stage(buf0, buf1, std::integral_constant<int, 3>(), step);
+        stage(buf1, buf0, std::integral_constant<int, 4>(), step);
+    }
+
+#pragma unroll
+    for (int q = 0; q < CPT; ++q) {
+        const int c = tid + q * RES_NT;
+        if (c < N) {
+            psi_g[c] = psi[q];
+            if (RES) n_g[c] = nn[q];
+        }
+    }
+    if (blockIdx.x == 0 && tid == 0) {
+        a.step_slots[0] = a.step0 + (uint64_t)a.n_steps;
+        a.step_slots[1] = a.step0 + (uint64_t)a.n_steps;
+    }
+}
+
+size_t resident_smem_bytes(int cells, int prec64) {
+    const size_t rb = prec64 ? 8 : 4;
+    return 2 * (size_t)(cells + 1) * 2 * rb + (size_t)cells * sizeof(ushort4) + 2 * (size_t)cells * rb;
+}
+
+// Cells per thread the instantiations cover (0 = the grid does not fit this variant).
+int resident_cpt(int cells, int prec64, bool res) {
+    const int max_cpt = (prec64 && res) ? 4 : 8;      // register budget of 128 per thread
+    const int need = (cells + RES_NT - 1) / RES_NT;
+    if (need > max_cpt || cells > 65534) return 0;
+    if (resident_smem_bytes(cells, prec64) > 227 * 1024) return 0;
+    return need <= 4 ? 4 : 8;
+}
+
+template <typename T, bool RES, bool NOISE, int CPT>
+static cudaError_t launch_one(const ResidentArgs<T>& a, cudaStream_t st) {
+    const size_t smem = resident_smem_bytes(a.geo.nx * a.geo.ny, sizeof(T) == 8);
+    auto kern = resident_kernel<T, RES, NOISE, CPT>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    kern<<<a.geo.batch, RES_NT, smem, st>>>(a);
+    return cudaGetLastError();
+}
+
+template <typename T>
+static cudaError_t launch_t(const ResidentArgs<T>& a, bool res, bool noise, cudaStream_t st) {
+    const int cpt = resident_cpt(a.geo.nx * a.geo.ny, sizeof(T) == 8, res);
+    if (cpt == 0) return cudaErrorInvalidConfiguration;
+#define PHX_RES_CASE(R, NZ)                                                      \
+    if (res == R && noise == NZ) {                                               \
+        if (cpt == 4) return launch_one<T, R, NZ, 4>(a, st);                     \
+        if constexpr (!(R && sizeof(T) == 8)) return launch_one<T, R, NZ, 8>(a, st); \
+    }
+    PHX_RES_CASE(false, false)
+    PHX_RES_CASE(false, true)
+    PHX_RES_CASE(true, false)
+    PHX_RES_CASE(true, true)
+#undef PHX_RES_CASE
+    return cudaErrorInvalidConfiguration;
+}
+
+cudaError_t launch_resident_32(const ResidentArgs<float>& a, bool res, bool noise, cudaStream_t st) { return launch_t<float>(a, res, noise, st); }
+cudaError_t launch_resident_64(const ResidentArgs<double>& a, bool res, bool noise, cudaStream_t st) { return launch_t<double>(a, res, noise, st); }
+
+}  // namespace phx

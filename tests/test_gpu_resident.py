@@ -1,0 +1,127 @@
+"""GPU parity of variant RESIDENT (a grid of at most 64 x 64 cells stays on chip for all steps of one launch;
+DESIGN.md section 5.3) against the CPU oracle, element by element, plus the invariants that need no oracle.
+Bars as everywhere (BASELINE.json north_star): relative L2 <= 1e-12 (complex fp64), <= 2e-5 (complex fp32)."""
+import dataclasses
+
+import numpy as np
+import pytest
+
+from paper_2411_18341_b200 import binding as phx
+from paper_2411_18341_b200 import workloads as wl
+from helpers import TOL, compare, make_gpu, make_oracle, rel_l2
+
+pytestmark = pytest.mark.gpu
+STAGE, STEP, RESIDENT = 1, 3, 4
+
+
+def run_pair(w, n_steps, **kw):
+    g = make_gpu(w, variant=RESIDENT, **kw)
+    assert g.get_variant() == RESIDENT
+    o = make_oracle(w, **{k: v for k, v in kw.items() if k in ("bc", "extra_params")})
+    g.step_rk4(n_steps)
+    o.step_rk4(n_steps)
+    errs = compare(g, o, w)
+    assert g.get_launch_count() == 1               # all steps in one launch
+    assert g.get_step() == n_steps
+    g.destroy()
+    return errs
+
+
+def test_cfg1_full_run():
+    w = wl.cfg1()                                  # 64 x 64, fp64, 1000 steps: BASELINE configs[0]
+    g = make_gpu(w, variant=RESIDENT)
+    assert g.get_variant() == RESIDENT
+    o = make_oracle(w)
+    g.step_rk4(w.n_steps)
+    o.step_rk4(w.n_steps)
+    errs = compare(g, o, w)
+    assert errs["psi_p"] <= 1e-12
+    g.destroy()
+
+
+@pytest.mark.parametrize("prec", ["c32", "c64"])
+@pytest.mark.parametrize("nx,ny", [(64, 64), (50, 41), (33, 7), (8, 5), (5, 4)])
+def test_scalar(prec, nx, ny):
+    run_pair(wl.cfg2(n=nx, ny=ny, prec=prec), 101)
+
+
+@pytest.mark.parametrize("prec,n", [("c32", 64), ("c32", 37), ("c64", 45), ("c64", 20)])
+def test_reservoir(prec, n):
+    run_pair(wl.cfg3(n=n, prec=prec), 200)
+
+
+@pytest.mark.parametrize("bc", [(1, 1), (1, 0), (0, 1)])
+@pytest.mark.parametrize("prec", ["c32", "c64"])
+def test_zero_boundaries_and_anisotropic_grid(bc, prec):
+    w = wl.cfg2(n=52, ny=31, prec=prec)
+    run_pair(dataclasses.replace(w, dy=w.dx * 1.3), 60, bc=bc)
+
+
+def test_density_offset():
+    run_pair(wl.cfg2(n=48, ny=32, prec="c64"), 50, extra_params=dict(density_offset=0.02))
+
+
+@pytest.mark.parametrize("prec", ["c32", "c64"])
+def test_noisy_ensemble(prec):
+    w = wl.cfg5(n=48 if prec == "c32" else 40, batch=33, prec=prec)
+    g = make_gpu(w)
+    assert g.get_variant() == RESIDENT             # AUTO: an ensemble (batch >= 32) of grids that fit
+    o = make_oracle(w)
+    g.step_rk4(40)
+    o.step_rk4(40)
+    compare(g, o, w)
+    assert rel_l2(g.ensemble_mean_density("psi_p"), o.ensemble_mean_density("psi_p")) <= TOL[prec]
+    g.destroy()
+
+
+def test_step_splitting_checkpoint_and_variant_switches_are_consistent():
+    w = wl.cfg5(n=40, batch=3)
+    g1, g2 = make_gpu(w, variant=RESIDENT), make_gpu(w, variant=RESIDENT)
+    g1.step_rk4(23)
+    for n in (1, 8, 9, 5):
+        g2.step_rk4(n)
+    for k in w.fields:                             # the step counter keys the noise: k calls of one step == one call of k
+        assert np.array_equal(g1.read_field(k), g2.read_field(k))
+    # RESIDENT -> STEP (odd number of steps: ping-pong parity) -> RESIDENT -> STAGE, against the oracle
+    g1.select_variant(STEP)
+    g1.step_rk4(3)
+    g1.select_variant(RESIDENT)
+    g1.step_rk4(4)
+    g1.select_variant(STAGE)
+    g1.step_rk4(2)
+    o = make_oracle(w)
+    o.step_rk4(32)
+    compare(g1, o, w)
+    assert g1.get_step() == 32
+    g1.destroy()
+    g2.destroy()
+
+
+def test_resident_agrees_with_step_to_rounding():
+    w = wl.cfg3(n=44, prec="c64")
+    a, b = make_gpu(w, variant=RESIDENT), make_gpu(w, variant=STEP)
+    a.step_rk4(50)
+    b.step_rk4(50)
+    for k in w.fields:
+        assert rel_l2(a.read_field(k), b.read_field(k)) <= 1e-13
+    a.destroy()
+    b.destroy()
+
+
+def test_grids_that_do_not_fit_are_refused():
+    for w, kw in ((wl.cfg2(n=128, ny=64, prec="c32"), {}), (wl.cfg4(n=32, prec="c32", sigma_cells=5.0), {}),
+                  (wl.cfg3(n=64, prec="c64"), {})):   # too many cells; spinor; fp64 reservoir beyond 2048 cells
+        g = make_gpu(w, **kw)
+        assert g.get_variant() == STEP
+        with pytest.raises(phx.PhxError) as e:
+            g.select_variant(RESIDENT)
+        assert e.value.status == phx.PHX_ERR_UNSUPPORTED
+        g.destroy()
+    w = wl.cfg2(n=32, ny=32, prec="c32")
+    g = make_gpu(w)
+    assert g.get_variant() == STEP                 # AUTO: a single small grid is faster spread over several SMs
+    g.select_variant(RESIDENT)
+    assert g.get_variant() == RESIDENT
+    g.set_drive(np.zeros((32, 32), np.complex64))  # a drive: the fused step takes over
+    assert g.get_variant() == STEP
+    g.destroy()

@@ -50,7 +50,7 @@ def build_workload(name):
     return table[name]()
 
 
-def algo_bytes_per_cell_step(w, variant):
+def algo_bytes_per_cell_step(w, variant, steps_per_launch=1):
     """Algorithmic HBM bytes per cell-step of variant STAGE, counted array by array.
 
     Per complex component: s1 R psi, W y2; s2 R y2, psi, W y3, acc; s3 R y3, psi, acc, W y4, acc;
@@ -59,6 +59,9 @@ def algo_bytes_per_cell_step(w, variant):
     rb = 8 if w.prec == "c64" else 4
     ncomp = 2 if w.model.startswith("spinor") else 1
     res = w.model.endswith("reservoir")
+    if variant == 4:
+        # variant RESIDENT: the same arrays once per LAUNCH (all steps of the call run on chip)
+        return algo_bytes_per_cell_step(w, 3) / max(1, steps_per_launch)
     if variant == 3:
         # variant STEP: every state array is read once and written once per step; V, P read once
         b = ncomp * 2 * 2 * rb + (ncomp * 2 * rb if res else 0)
@@ -325,17 +328,18 @@ def main():
 
     # ---- roofline of the dominant kernel ------------------------------------------------------------------------
     peak, peak_src = measured_peaks()
-    bpc = algo_bytes_per_cell_step(w, variant)
+    bpc = algo_bytes_per_cell_step(w, variant, args.steps)
     kernels_per_step = launches / args.steps
     bytes_per_launch = bpc * cells / kernels_per_step
     launch_ms = ms / launches
     achieved = bytes_per_launch / (launch_ms * 1e-3) / 1e9
     comp = COMPULSORY_BYTES[w.model] * (2 if w.prec == "c64" else 1)
-    kernel = {1: "phx::stage_kernel (4 launches per step)", 3: "phx::step_kernel (1 launch per step)"}.get(variant, str(variant))
+    kernel = {1: "phx::stage_kernel (4 launches per step)", 3: "phx::step_kernel (1 launch per step)",
+              4: "phx::resident_kernel (1 launch for all steps)"}.get(variant, str(variant))
     hbm = {"achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "peak_source": peak_src,
            "algorithmic_bytes_per_cell_step": bpc, "bytes_per_launch": bytes_per_launch,
            "compulsory_bytes_per_cell_step": comp, "compulsory_frac": value / world * 1e9 * comp / 1e9 / peak}
-    if variant == phx.PHX_VARIANT_STEP:
+    if variant in (phx.PHX_VARIANT_STEP, phx.PHX_VARIANT_RESIDENT):
         # the fused step moves the compulsory bytes only; it is bound by plain FP32/FP64 instruction issue
         fpc = algo_flops_per_cell_step(w)
         alu_peak = ALU_PEAK_TFLOPS[w.prec]

@@ -98,3 +98,55 @@ def test_cfg5_full_ensemble():
     mean = g.ensemble_mean_density("psi_p")
     assert rel_l2(mean, o.ensemble_mean_density("psi_p")) <= TOL["c32"]
     g.destroy()
+
+
+# ---- late segments: the oracle restarted from a GPU checkpoint far into the run (SURVEY.md 8(c) "horizons") ----------
+def _check_windows_from_checkpoint(w, n_before, corners):
+    """Steps the GPU n_before steps, checkpoints, steps S more; the oracle redoes the S steps from the checkpoint."""
+    import dataclasses
+    g = make_gpu(w)
+    g.step_rk4(n_before)
+    snap = {name: g.read_field(name) for name in w.fields}
+    for name, arr in snap.items():
+        assert np.all(np.isfinite(arr)), name
+    g.step_rk4(S)
+    got = {name: g.read_field(name) for name in w.fields}
+    g.destroy()
+    w2 = dataclasses.replace(w, fields=snap)
+    for (x0, y0) in corners:
+        ref = _window_oracle(w2, x0, y0)
+        ix, iy = np.arange(x0, x0 + WIN) % w.nx, np.arange(y0, y0 + WIN) % w.ny
+        for name in w.fields:
+            err = rel_l2(got[name][0][np.ix_(iy, ix)], ref[name])
+            assert err <= TOL[w.prec], f"{w.name} {name} window ({x0},{y0}) after {n_before} steps: rel L2 {err:.3e}"
+
+
+def test_cfg2_4096_segment_at_step_5000():
+    _check_windows_from_checkpoint(wl.cfg2(n=4096, prec="c32"), 5000, _corners(4096))
+
+
+def test_cfg3_4096_segment_at_step_10000():
+    # the pumped reservoir has built up and the condensate has grown by then (n0 = 0, psi0 = noise at the start)
+    _check_windows_from_checkpoint(wl.cfg3(n=4096, prec="c32"), 10000, _corners(4096))
+
+
+def test_cfg5_last_steps_of_the_run():
+    w = wl.cfg5(n=256, batch=512, prec="c32")
+    n_before, n_last = w.n_steps - 2, 2          # steps 19 998 and 19 999 of the 20 000
+    g = make_gpu(w)
+    g.step_rk4(n_before)
+    snap = {name: g.read_field(name) for name in w.fields}
+    g.step_rk4(n_last)
+    assert g.get_step() == w.n_steps
+    o = orc.Oracle(w.nx, w.ny, w.dx, w.dy, orc.make_params(**w.params), model=w.model, batch=w.batch, prec32=True,
+                   noise=True, seed=w.seed, P=w.P.astype(np.float64))
+    for name, arr in snap.items():
+        assert np.all(np.isfinite(arr)), name
+        o.set_field(name, arr)
+    o.step = n_before                            # the step index keys the noise
+    o.step_rk4(n_last)
+    for name in w.fields:
+        got, ref = g.read_field(name), getattr(o, name)
+        worst = max(rel_l2(got[r], ref[r]) for r in range(w.batch))
+        assert worst <= TOL["c32"], f"{name}: worst realisation rel L2 {worst:.3e}"
+    g.destroy()

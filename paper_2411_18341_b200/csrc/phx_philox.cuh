@@ -42,4 +42,24 @@ __device__ __forceinline__ double2 normal_pair(uint32_t w0, uint32_t w1, double)
     return make_double2(rad * c, rad * s);
 }
 
+// The noise increment of one cell, Eq. (22): sqrt(var) (xi_1 + i xi_2) with var the variance per real component, as ONE
+// square root: sqrt(-2 ln(u1) var) (cos, sin)(2 pi u2).
+__device__ __forceinline__ float2 noise_increment(uint32_t w0, uint32_t w1, float var) {
+    const float u1 = ((float)(w0 >> 9) + 0.5f) * 1.1920928955078125e-07f;
+    const float u2 = ((float)(w1 >> 9) + 0.5f) * 1.1920928955078125e-07f;
+    const float amp = sqrtf(-2.0f * logf(u1) * var);
+    float s, c;
+    sincospif(2.0f * u2, &s, &c);
+    return make_float2(amp * c, amp * s);
+}
+
+__device__ __forceinline__ double2 noise_increment(uint32_t w0, uint32_t w1, double var) {
+    const double u1 = ((double)(w0 >> 9) + 0.5) * 1.1920928955078125e-07;
+    const double u2 = ((double)(w1 >> 9) + 0.5) * 1.1920928955078125e-07;
+    const double amp = sqrt(-2.0 * log(u1) * var);
+    double s, c;
+    sincospi(2.0 * u2, &s, &c);
+    return make_double2(amp * c, amp * s);
+}
+
 }  // namespace phx

@@ -98,10 +98,8 @@ resident_kernel(const __grid_constant__ ResidentArgs<T> a) {
                     C nw = fma2s(w_dt, K, acc[q]);
                     if (NOISE) {
                         const uint4 wd = noise_words(a.seed, blockIdx.x, step, (uint32_t)c);
-                        const C xi = normal_pair(wd.x, wd.y, T(0));
                         const T nt = RES ? nn[q] : T(0);          // reservoir at the start of the step
-                        const T sigma = sqrt(k.sig2 * (T(2) * k.hgc + k.Rr * nt));
-                        nw = fma2s(sigma, xi, nw);
+                        nw = add2(nw, noise_increment(wd.x, wd.y, k.sig2 * (T(2) * k.hgc + k.Rr * nt)));
                     }
                     psi[q] = nw;
                     if (RES) nn[q] = nacc[q] + w_dt * Kn;

@@ -450,10 +450,9 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
                             for (int i = 0; i < VEC; ++i) {
                                 const uint32_t cell = (uint32_t)jr * (uint32_t)nx + (uint32_t)(xl + i);
                                 const uint4 wd = noise_words(a.seed, blockIdx.z, step, cell);
-                                const C xi = s == 0 ? normal_pair(wd.x, wd.y, T(0)) : normal_pair(wd.z, wd.w, T(0));
                                 const T nt = RES ? nr[s][SL(-3)][i] : T(0);      // reservoir at the start of the step
-                                const T sigma = sqrt(k.sig2 * (T(2) * k.hgc + k.Rr * nt));
-                                out[i] = fma2s(sigma, xi, out[i]);
+                                const T var = k.sig2 * (T(2) * k.hgc + k.Rr * nt);
+                                out[i] = add2(out[i], s == 0 ? noise_increment(wd.x, wd.y, var) : noise_increment(wd.z, wd.w, var));
                             }
                         }
                         stc<VEC>(pout[s] + est, out);

@@ -298,7 +298,7 @@ int step_rows_per_chunk(const phx_grid* g, int vec) {
         const int real_chunks = (g->d.ny + ly - 1) / ly;
         const long ctas = ctas_row * real_chunks;
         const long waves = (ctas + slots - 1) / slots;
-        const long iters = (ly + 6 + 4) / 5 * 5;
+        const long iters = (ly + 6 + PHX_STEP_RING - 1) / PHX_STEP_RING * PHX_STEP_RING;
         double cost = (double)(waves * iters);
         if (in_l2) {
             const long per_sm = ((ctas + waves - 1) / waves + g->n_sm - 1) / g->n_sm;     // CTAs on the fullest SM

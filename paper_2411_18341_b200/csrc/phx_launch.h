@@ -8,6 +8,13 @@
 #define PHX_STEP_WARPS 2
 #endif
 
+// Variant STEP: row iterations a fetch leads its first use by, and the ring length / unroll factor of the row loop.
+// (LEAD = 2 costs registers and is slower everywhere: 200.6 against 207.5 Gcell*step/s at 4096^2 fp32, spills in the spinor.)
+#ifndef PHX_STEP_LEAD
+#define PHX_STEP_LEAD 1
+#endif
+#define PHX_STEP_RING (4 + PHX_STEP_LEAD)
+
 namespace phx {
 
 template <typename T> struct StageArgs;

@@ -134,8 +134,8 @@ __device__ __forceinline__ void gather(const typename Cx<T>::type (&rs)[VEC], co
 // Rows carried in registers live in RINGS of PHX_STEP_RING slots: the row with number q sits in slot q mod RING of
 // its ring for as long as it is live, and the row loop is unrolled RING times, so that every slot index is a
 // compile-time constant and moving the windows down by one row costs no instruction (a dead slot costs no
-// register either).  RING = 5 is the longest life: psi rows j-2 .. j+2 and V rows j-3 .. j+1.
-#define PHX_STEP_RING 5
+// register either).  RING = 4 + LEAD is the longest life: psi rows j-2 .. j+1+LEAD and V rows j-3 .. j+LEAD, where LEAD
+// (PHX_STEP_LEAD, phx_launch.h) is the number of row iterations a fetch leads its first use by.
 
 // MINW: resident warps per SM the register budget is sized for.  ISO: dx == dy (scalar and reservoir models only).
 // DRIVE: coherent drive E(r) exp(-i omega t) (reading Q17), shared by both components.
@@ -148,7 +148,7 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
     constexpr bool RES = model_reservoir(MODEL);
     constexpr int NC = SPINOR ? 2 : 1;
     constexpr int W = 32 * VEC, OUTW = W - 8;
-    constexpr int RING = PHX_STEP_RING;
+    constexpr int RING = PHX_STEP_RING, LEAD = PHX_STEP_LEAD;
     const Geom& g = a.geo;
     const Coef<T>& k = a.k;
     const int nx = g.nx, ny = g.ny;
@@ -271,14 +271,14 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
 
     // ---- pipeline fill: psi rows j0-1, j0, j0+1 and the row-local inputs (V, P, n) of row j0 ----------------------------------
 #pragma unroll
-    for (int d = -1; d <= 1; ++d) {
+    for (int d = -1; d <= LEAD; ++d) {
         constexpr int R2 = 2 * RING;
         const bool okq = !ZBC || (inx && (!zy || (qw >= 0 && qw < ny)));
 #pragma unroll
         for (int s = 0; s < NC; ++s) {
             if (okq) ldc<VEC>(pin[s] + ew, psr[s][(d + R2) % RING]);
         }
-        if (d == 0 && okq) {
+        if (d >= 0 && d < LEAD && okq) {
             if (Vp) ldr<VEC>(Vp + ew, Vr[(d + R2) % RING]);
             if (Pp) ldr<VEC>(Pp + ew, Pr[(d + R2) % RING]);
             if (DRIVE) ldc<VEC>(Ep + ew, Er[(d + R2) % RING]);
@@ -313,7 +313,7 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
                     if (Vp) prefetch_l2(Vp + e);
                     if (Pp) prefetch_l2(Pp + e);
                     if (DRIVE) prefetch_l2(Ep + e);
-                } else if (inx && (j + 2 + pfr <= r1 + 3) && qw + pfr < ny && qw + pfr >= 0) {
+                } else if (inx && (j + 1 + LEAD + pfr <= r1 + 3) && qw + pfr < ny && qw + pfr >= 0) {
 #pragma unroll
                     for (int s = 0; s < NC; ++s) {
                         prefetch_l2(pin[s] + ew + epf);
@@ -327,32 +327,32 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
             // ---- fetch: psi row j+2; row-local inputs (V, P, n) of row j+1 -------------------------------------------------
             // Periodic: every (wrapped) row is readable, so the fetch is unconditional (rows past r1+3 are fetched and not
             // used).  Zero boundaries: a row or column outside the grid reads as 0.
-            const bool okq = !ZBC || (inx && (j + 2 <= r1 + 3) && (!zy || (qw >= 0 && qw < ny)));
+            const bool okq = !ZBC || (inx && (j + 1 + LEAD <= r1 + 3) && (!zy || (qw >= 0 && qw < ny)));
 #pragma unroll
             for (int s = 0; s < NC; ++s) {
                 if (ZBC) {
 #pragma unroll
-                    for (int i = 0; i < VEC; ++i) psr[s][SL(2)][i] = czero;
+                    for (int i = 0; i < VEC; ++i) psr[s][SL(1 + LEAD)][i] = czero;
                 }
-                if (okq) ldc<VEC>(pin[s] + ew, psr[s][SL(2)]);
+                if (okq) ldc<VEC>(pin[s] + ew, psr[s][SL(1 + LEAD)]);
             }
             if (ZBC) {              // (periodic without V or P: the slots keep the zeros they were initialised with)
 #pragma unroll
-                for (int i = 0; i < VEC; ++i) { Vr[SL(1)][i] = T(0); Pr[SL(1)][i] = T(0); Er[SL(1)][i] = czero; }
+                for (int i = 0; i < VEC; ++i) { Vr[SL(LEAD)][i] = T(0); Pr[SL(LEAD)][i] = T(0); Er[SL(LEAD)][i] = czero; }
             }
             if (okprev) {
-                if (Vp) ldr<VEC>(Vp + ewp, Vr[SL(1)]);
-                if (Pp) ldr<VEC>(Pp + ewp, Pr[SL(1)]);
-                if (DRIVE) ldc<VEC>(Ep + ewp, Er[SL(1)]);
+                if (Vp) ldr<VEC>(Vp + ewp, Vr[SL(LEAD)]);
+                if (Pp) ldr<VEC>(Pp + ewp, Pr[SL(LEAD)]);
+                if (DRIVE) ldc<VEC>(Ep + ewp, Er[SL(LEAD)]);
             }
             if constexpr (RES) {
 #pragma unroll
                 for (int s = 0; s < NC; ++s) {
                     if (ZBC) {
 #pragma unroll
-                        for (int i = 0; i < VEC; ++i) nr[s][SL(1)][i] = T(0);
+                        for (int i = 0; i < VEC; ++i) nr[s][SL(LEAD)][i] = T(0);
                     }
-                    if (okprev) ldr<VEC>(nin[s] + ewp, nr[s][SL(1)]);
+                    if (okprev) ldr<VEC>(nin[s] + ewp, nr[s][SL(LEAD)]);
                 }
             }
 

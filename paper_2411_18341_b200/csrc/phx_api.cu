@@ -292,7 +292,7 @@ int step_rows_per_chunk(const phx_grid* g, int vec) {
     const bool in_l2 = plane_cells(g) * g->d.batch * step_bytes_per_cell(g) < g->l2_bytes / 2;
     double best_cost = -1;
     int best_ly = g->d.ny;
-    const int max_chunks = g->d.ny / 8 > 0 ? g->d.ny / 8 : 1;
+    const int max_chunks = g->d.ny / 4 > 0 ? g->d.ny / 4 : 1;   // (a 64^2 grid: ly = 4, 3.6 instead of 4.9 us per step)
     for (int nch = 1; nch <= max_chunks && nch <= 65535; ++nch) {
         const int ly = (g->d.ny + nch - 1) / nch;
         const int real_chunks = (g->d.ny + ly - 1) / ly;

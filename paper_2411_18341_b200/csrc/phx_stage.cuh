@@ -144,8 +144,11 @@ struct AuxShared {
     typename Cx<T>::type E[VEC];
 };
 
+#ifndef PHX_STAGE_MINB_SPINOR
+#define PHX_STAGE_MINB_SPINOR 4
+#endif
 template <typename T, int VEC, int MODEL, int STAGE, bool NOISE>
-__global__ void __launch_bounds__(128)
+__global__ void __launch_bounds__(128, (model_spinor(MODEL) && sizeof(T) == 4) ? PHX_STAGE_MINB_SPINOR : 1)
 stage_kernel(const __grid_constant__ StageArgs<T> a) {
     using C = typename Cx<T>::type;
     constexpr bool SPINOR = model_spinor(MODEL);

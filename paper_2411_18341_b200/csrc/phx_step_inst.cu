@@ -26,6 +26,9 @@ typedef double real_t;
 #define PHX_MINW_V2 8
 #define PHX_MINW_V1 (PHX_INST_MODEL == 0 ? 16 : (PHX_INST_MODEL == 1 ? 12 : 8))
 #endif
+#ifndef PHX_MINW_V4
+#define PHX_MINW_V4 8
+#endif
 // The isotropic form of the Laplacian exists for the models without TE-TM coupling.
 #define PHX_HAS_ISO (PHX_INST_MODEL < 2)
 // Four cells per lane (two 128-bit loads): complex fp32, scalar model only (the other models run out of registers).
@@ -40,7 +43,7 @@ typedef double real_t;
 template <int VEC, bool NOISE, bool ZBC, bool ISO, bool DRIVE>
 struct Inst {
     // (the noisy reservoir kernel, cfg5, is 9 % faster with the registers of 8 resident warps than with those of 12)
-    static constexpr int MINW = VEC == 4 ? 8 : (VEC == 2 ? ((NOISE && PHX_INST_MODEL == 1 && PHX_INST_PREC == 32) ? 8 : PHX_MINW_V2) : PHX_MINW_V1);
+    static constexpr int MINW = VEC == 4 ? PHX_MINW_V4 : (VEC == 2 ? ((NOISE && PHX_INST_MODEL == 1 && PHX_INST_PREC == 32) ? 8 : PHX_MINW_V2) : PHX_MINW_V1);
     static constexpr bool I = ISO && PHX_HAS_ISO;
     static cudaError_t launch(const StepArgs<real_t>& a, dim3 grid, cudaStream_t st) {
         step_kernel<real_t, VEC, PHX_INST_MODEL, NOISE, ZBC, I, DRIVE, MINW><<<grid, 32 * PHX_STEP_WARPS, 0, st>>>(a);

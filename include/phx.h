@@ -151,7 +151,10 @@ phx_status phx_select_variant(phx_grid* g, int32_t variant);
 /* Bench/test aids: the variant the next phx_step_rk4 will use; kernels launched so far by this handle;
  * launch geometry knobs (key/value, UNSUPPORTED for unknown keys): "rows", "vec" (variant STAGE: rows per
  * CTA, cells per thread), "step_ly", "step_vec" (variant STEP: rows per chunk, cells per lane; 0 = automatic),
- * "graph_steps" (RK4 steps per captured CUDA graph).  Results do not depend on them. */
+ * "graph_steps" (RK4 steps per captured CUDA graph).  Results do not depend on them.
+ * "async_host_copies" = 1: phx_set_field / phx_read_field with PHX_HOST enqueue the copy on the stream and return
+ * without synchronising (the host buffers must be pinned and stay untouched until phx_sync); lets a caller overlap the
+ * upload of one grid with the download of another on two handles / streams. */
 phx_status phx_get_variant(const phx_grid* g, int32_t* variant);
 phx_status phx_get_launch_count(const phx_grid* g, uint64_t* launches);
 phx_status phx_set_tuning(phx_grid* g, const char* key, int32_t value);

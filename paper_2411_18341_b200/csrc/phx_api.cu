@@ -87,6 +87,7 @@ struct phx_grid {
     int rows, vec, graph_steps, gsteps;
     int parity;             // variant STEP ping-pongs the state: 0 = state in psi/n, 1 = state in ya/na
     int step_ly, step_vec;  // variant STEP geometry (0 = automatic)
+    int async_host;         // 1: host copies of set_field / read_field do not synchronise (pinned buffers, caller syncs)
     cudaGraphExec_t g1[2], gN;  // one step from parity 0 / 1; graph_steps steps from parity 0
     bool graphs_valid;
     int n_sm;
@@ -460,7 +461,7 @@ phx_status apply_variant(phx_grid* g) {
 phx_status copy_in(phx_grid* g, void* dst, const void* src, size_t bytes, phx_mem where) {
     if (where == PHX_HOST) {
         PHX_CUDA(g, cudaMemcpyAsync(dst, src, bytes, cudaMemcpyHostToDevice, g->stream));
-        PHX_CUDA(g, cudaStreamSynchronize(g->stream));   // the caller may reuse a pageable source at once
+        if (!g->async_host) PHX_CUDA(g, cudaStreamSynchronize(g->stream));   // the caller may reuse a pageable source at once
     } else {
         PHX_CUDA(g, cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToDevice, g->stream));
     }
@@ -470,7 +471,7 @@ phx_status copy_in(phx_grid* g, void* dst, const void* src, size_t bytes, phx_me
 phx_status copy_out(phx_grid* g, void* dst, const void* src, size_t bytes, phx_mem where) {
     PHX_CUDA(g, cudaMemcpyAsync(dst, src, bytes, where == PHX_HOST ? cudaMemcpyDeviceToHost : cudaMemcpyDeviceToDevice,
                                 g->stream));
-    PHX_CUDA(g, cudaStreamSynchronize(g->stream));
+    if (!(g->async_host && where == PHX_HOST)) PHX_CUDA(g, cudaStreamSynchronize(g->stream));
     return PHX_OK;
 }
 
@@ -522,6 +523,7 @@ phx_status phx_create_grid(phx_grid** out, const phx_grid_desc* desc) {
     g->graphs_valid = false;
     g->parity = 0;
     g->step_ly = g->step_vec = 0;
+    g->async_host = 0;
     g->n_sm = prop.multiProcessorCount;
     g->l2_bytes = (size_t)prop.l2CacheSize;
     g->sticky = cudaSuccess;
@@ -760,6 +762,10 @@ phx_status phx_set_tuning(phx_grid* g, const char* key, int32_t value) {
         if (value == 4 && (g->d.model != PHX_SCALAR || g->d.prec != PHX_C32)) return fail(g, PHX_ERR_UNSUPPORTED, "step_vec=4 exists for the scalar fp32 model only");
         if (value == 2 && g->d.prec == PHX_C64 && g->d.model != PHX_SCALAR) return fail(g, PHX_ERR_UNSUPPORTED, "step_vec=2 in fp64 exists for the scalar model only");
         g->step_vec = value;
+    } else if (!std::strcmp(key, "async_host_copies")) {   // 1: phx_set_field / phx_read_field with PHX_HOST do not synchronise
+        if (value != 0 && value != 1) return PHX_ERR_INVALID_ARG;
+        g->async_host = value;
+        return PHX_OK;                                 // (no effect on the launch plan: keep the captured graphs)
     } else if (!std::strcmp(key, "graph_steps")) {
         if (value < 1 || value > 256) return PHX_ERR_INVALID_ARG;
         g->graph_steps = value;

@@ -280,3 +280,29 @@ def test_step_and_stage_agree_to_rounding():
         assert rel_l2(a.read_field(k), b.read_field(k)) <= 1e-13
     a.destroy()
     b.destroy()
+
+
+def test_async_host_copies_give_the_same_bits():
+    # "async_host_copies": set_field / read_field enqueue the copy and return; phx_sync fences (bench.py's end-to-end leg)
+    import torch
+    w = wl.cfg2(n=300, ny=70, prec="c32")
+    g = make_gpu(w, variant=STEP)
+    g.step_rk4(3)
+    ref = g.read_field("psi_p")
+    g.destroy()
+    pin_in = torch.from_numpy(np.ascontiguousarray(w.fields["psi_p"])).pin_memory()
+    handles = [make_gpu(w, variant=STEP) for _ in range(2)]
+    outs = [torch.empty_like(pin_in).pin_memory() for _ in handles]
+    for h in handles:
+        h.set_tuning("async_host_copies", 1)
+    for rep in range(3):
+        for h, out in zip(handles, outs):
+            h.sync()
+            h.set_field("psi_p", pin_in)
+            h.set_step(0)
+            h.step_rk4(3)
+            h.read_field("psi_p", out)
+    for h, out in zip(handles, outs):
+        h.sync()
+        assert np.array_equal(out.numpy().reshape(ref.shape), ref)
+        h.destroy()

@@ -111,23 +111,36 @@ size_t phx_workspace_bytes(const phx_grid_desc* desc);
  * Errors: INVALID_ARG, WORKSPACE, CUDA (no device / not sm_100). *out is NULL on error. */
 phx_status phx_create_grid(phx_grid** out, const phx_grid_desc* desc);
 
-/* Sets the physical parameters and derives the canonical coefficient set (rounded once to T).
- * May return PHX_WARN_UNSTABLE (parameters are set nevertheless). */
+/* Sets the physical parameters of Eq. (1) (hbar, m, g, gamma), Eq. (16) (g_x, g_r, R, Delta_LT,
+ * drive frequency), Eq. (17) (gamma_r, R) and Eq. (22) (noise scale nu, 1/DeltaV of the
+ * renormalised density :452) and the RK4 step dt of Eqs. (2)-(6), and derives the canonical coefficient set
+ * (DESIGN.md section 2 step 0: double expressions, each rounded once to T).  Invalidates the captured graphs.
+ * Errors: INVALID_ARG (NULL, dt <= 0, hbar or m zero or non-finite, a non-finite coefficient).  May return
+ * PHX_WARN_UNSTABLE (the explicit scheme is unstable for these values; the parameters are set nevertheless). */
 phx_status phx_set_params(phx_grid* g, const phx_params* p);
 
-/* Static real fields [ny][nx] of type T shared by the batch: potential V (Eq. (1)) and pump P
- * (Eq. (17), P_+ = P_-).  NULL = identically zero.  The data are copied into the workspace. */
+/* Static real fields [ny][nx] of type T shared by the batch: potential V (Eq. (1), PAPER.md:25) and pump P
+ * (Eq. (17); P_+ = P_-, reading Q18).  NULL = identically zero.  The data are copied into the
+ * workspace; the caller keeps its arrays.  UNSUPPORTED: P given for a model without reservoir. */
 phx_status phx_set_potential_pump(phx_grid* g, const void* V, const void* P, phx_mem where);
 
 /* Complex drive amplitude E(r) [ny][nx] (Eq. (16), E_+ = E_-); NULL = no drive. */
 phx_status phx_set_drive(phx_grid* g, const void* E, phx_mem where);
 
-/* Copies a state field [batch][ny][nx] into / out of the workspace.  phx_read_field synchronises
- * the stream before returning.  UNSUPPORTED if the model does not have the field. */
+/* Copies a state field [batch][ny][nx] into / out of the workspace: psi_+- of Eq. (16) (PHX_PSI alone is
+ * psi of Eq. (1)) as interleaved complex T, the reservoirs n_+- of Eq. (17) as real T.
+ * The caller keeps ownership of src / dst (host or device, see phx_mem).  phx_read_field synchronises the stream before
+ * returning (unless "async_host_copies" is set, see phx_set_tuning).  Together with phx_get_step / phx_set_step the fields
+ * are a complete checkpoint.  INVALID_ARG: NULL pointer or bad enum; UNSUPPORTED: the model does not have the field. */
 phx_status phx_set_field(phx_grid* g, phx_field f, const void* src, phx_mem where);
 phx_status phx_read_field(phx_grid* g, phx_field f, void* dst, phx_mem where);
 
-/* Advances every realisation by n_steps (>= 0) RK4 steps.  Asynchronous on the stream. */
+/* Advances every realisation by n_steps (>= 0) fixed-step RK4 steps, Eqs. (2)-(6) with the weights of
+ * Listing 1, on the joint state (psi_+-, n_+-) (reading Q5); each step evaluates the
+ * derivative of Eq. (1)/(16)/(17) four times (Laplacian Eq. (8)) and, with noise = 1, adds the Wiener
+ * increment of Eq. (22) after the step.  All of it runs in the kernels of the selected variant,
+ * replayed from CUDA graphs; asynchronous on the stream, no host synchronisation.
+ * INVALID_ARG: n_steps < 0; BAD_STATE: phx_set_params not called yet; CUDA: a launch failed (sticky). */
 phx_status phx_step_rk4(phx_grid* g, int64_t n_steps);
 
 /* Step counter = number of completed steps.  phx_set_step synchronises. */
@@ -140,8 +153,10 @@ phx_status phx_ensemble_mean_density(phx_grid* g, phx_field f, void* dst, phx_me
 /* The canonical coefficients actually used (as double); n must be PHX_NCOEF. */
 phx_status phx_get_coeffs(const phx_grid* g, double* out, int32_t n);
 
-/* Test aid: the four Philox4x32-10 words every (realisation, cell) draws at step `step`,
- * dst[batch][ny][nx][4], produced by the same device function the stepping kernels call. */
+/* Test aid: the four Philox4x32-10 words every (realisation, cell) draws at step `step` for the noise of Eq. (22)
+ * (BASELINE.json config 5: keyed by (seed, realisation, step, cell); counter/key packing of DESIGN.md
+ * reading Q13), dst[batch][ny][nx][4] (host or device, caller-owned), produced by the same device function the stepping
+ * kernels call.  Synchronises.  BAD_STATE before phx_set_params (the seed is a parameter). */
 phx_status phx_debug_noise_u32(phx_grid* g, uint64_t step, uint32_t* dst, phx_mem where);
 
 /* Selects a kernel variant (phx_variant).  UNSUPPORTED if it cannot run this grid/model.  All variants

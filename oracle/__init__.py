@@ -26,7 +26,7 @@ class _Problem(C.Structure):
     _fields_ = [("nx", C.c_int32), ("ny", C.c_int32), ("batch", C.c_int32), ("spinor", C.c_int32),
                 ("reservoir", C.c_int32), ("noise", C.c_int32), ("bc_x", C.c_int32), ("bc_y", C.c_int32),
                 ("seed", C.c_uint32), ("coef", C.c_double * NCOEF), ("V", C.c_void_p), ("P", C.c_void_p),
-                ("E", C.c_void_p)]
+                ("E", C.c_void_p), ("first_realisation", C.c_uint32)]
 
 
 _lib = None
@@ -81,7 +81,7 @@ class Oracle:
     """
 
     def __init__(self, nx, ny, dx, dy, params, model="scalar", batch=1, prec32=False, noise=False, seed=0,
-                 bc=(0, 0), V=None, P=None, E=None, coef=None):
+                 bc=(0, 0), V=None, P=None, E=None, coef=None, first_realisation=0):
         self.nx, self.ny, self.batch = int(nx), int(ny), int(batch)
         self.model = model
         self.spinor = model in ("spinor", "spinor_reservoir")
@@ -94,7 +94,7 @@ class Oracle:
         self.E = None if E is None else np.ascontiguousarray(E, dtype=np.complex128).reshape(ny, nx)
         self.pb = _Problem(self.nx, self.ny, self.batch, int(self.spinor), int(self.reservoir), int(bool(noise)),
                            int(bc[0]), int(bc[1]), int(seed), (C.c_double * NCOEF)(*self.coef), _ptr(self.V),
-                           _ptr(self.P), _ptr(self.E))
+                           _ptr(self.P), _ptr(self.E), int(first_realisation))
         shape = (self.batch, self.ny, self.nx)
         self.psi_p = np.zeros(shape, np.complex128)
         self.psi_m = np.zeros(shape, np.complex128) if self.spinor else None

@@ -270,7 +270,7 @@ int32_t orc_step_rk4(const orc_problem* pb, double* psi_p_, double* psi_m_, doub
             if (pb->noise) {
                 for (size_t k = 0; k < N; ++k) {
                     const uint32_t ctr[4] = {(uint32_t)k, (uint32_t)(step & 0xffffffffu), (uint32_t)(step >> 32), 0u};
-                    const uint32_t key[2] = {pb->seed, (uint32_t)r};
+                    const uint32_t key[2] = {pb->seed, pb->first_realisation + (uint32_t)r};
                     uint32_t w[4];
                     philox4x32_10(ctr, key, w);
                     for (int s = 0; s < ncomp; ++s) {

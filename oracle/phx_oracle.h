@@ -68,6 +68,8 @@ typedef struct {
     const double* V;             /* [ny][nx] real, shared by the batch; NULL = 0 */
     const double* P;             /* [ny][nx] real pump P_+ = P_-; NULL = 0 */
     const double* E;             /* [ny][nx] complex drive amplitude E_+ = E_-; NULL = 0 */
+    uint32_t first_realisation;  /* Philox key word 1 of batch element 0 (element r uses first_realisation + r), so
+                                    that single realisations of a large ensemble can be stepped on their own */
 } orc_problem;
 
 void orc_derive_coeffs(const orc_params* p, double dx, double dy, int32_t prec32,

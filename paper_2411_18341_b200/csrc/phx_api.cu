@@ -416,7 +416,7 @@ bool step_variant_ok(const phx_grid* g) {
 // Variant RESIDENT: scalar and reservoir models without drive whose grid fits one CTA (phx_resident.cu).
 bool resident_variant_ok(const phx_grid* g) {
     if (model_spinor(g->d.model) || g->hasE) return false;
-    return resident_cpt(g->d.nx * g->d.ny, g->d.prec == PHX_C64, model_reservoir(g->d.model)) != 0;
+    return resident_cpt(plane_cells(g), g->d.prec == PHX_C64, model_reservoir(g->d.model)) != 0;
 }
 
 // AUTO takes the resident kernel for ensembles of grids that fit it (one CTA per realisation: 2.3x the fused step on
@@ -451,7 +451,6 @@ phx_status normalise_state(phx_grid* g) {
 
 // Re-resolves the variant after a request or a change of the terms present; drops the captured graphs.
 phx_status apply_variant(phx_grid* g) {
-    const int before = g->variant;
     resolve_variant(g);
     drop_graphs(g);
     if (g->variant == PHX_VARIANT_STAGE) return normalise_state(g);   // STAGE keeps the state in psi/n
@@ -580,6 +579,8 @@ phx_status phx_set_params(phx_grid* g, const phx_params* p) {
 phx_status phx_set_potential_pump(phx_grid* g, const void* V, const void* P, phx_mem where) {
     if (!g || (where != PHX_HOST && where != PHX_DEVICE)) return PHX_ERR_INVALID_ARG;
     if (g->sticky != cudaSuccess) return PHX_ERR_CUDA;
+    if (P && !model_reservoir(g->d.model))
+        return fail(g, PHX_ERR_UNSUPPORTED, "phx_set_potential_pump: a pump P needs a model with a reservoir (Eq. (17))");
     const size_t bytes = plane_cells(g) * real_bytes(g);
     if (V) { phx_status s = copy_in(g, g->ws + g->L.V, V, bytes, where); if (s) return s; }
     if (P) { phx_status s = copy_in(g, g->ws + g->L.P, P, bytes, where); if (s) return s; }

@@ -60,7 +60,7 @@ struct ResidentArgs {
     int n_steps;
     uint32_t seed;
 };
-int resident_cpt(int cells, int prec64, bool res);     // cells per thread, 0 = the grid does not fit
+int resident_cpt(size_t cells, int prec64, bool res);     // cells per thread, 0 = the grid does not fit
 cudaError_t launch_resident_32(const ResidentArgs<float>&, bool res, bool noise, cudaStream_t);
 cudaError_t launch_resident_64(const ResidentArgs<double>&, bool res, bool noise, cudaStream_t);
 

@@ -138,11 +138,12 @@ size_t resident_smem_bytes(int cells, int prec64) {
 }
 
 // Cells per thread the instantiations cover (0 = the grid does not fit this variant).
-int resident_cpt(int cells, int prec64, bool res) {
+int resident_cpt(size_t cells, int prec64, bool res) {
+    if (cells > 65534) return 0;                      // neighbour indices are 16 bit
     const int max_cpt = (prec64 && res) ? 4 : 8;      // register budget of 128 per thread
-    const int need = (cells + RES_NT - 1) / RES_NT;
-    if (need > max_cpt || cells > 65534) return 0;
-    if (resident_smem_bytes(cells, prec64) > 227 * 1024) return 0;
+    const int need = ((int)cells + RES_NT - 1) / RES_NT;
+    if (need > max_cpt) return 0;
+    if (resident_smem_bytes((int)cells, prec64) > 227 * 1024) return 0;
     return need <= 4 ? 4 : 8;
 }
 
@@ -158,7 +159,7 @@ static cudaError_t launch_one(const ResidentArgs<T>& a, cudaStream_t st) {
 
 template <typename T>
 static cudaError_t launch_t(const ResidentArgs<T>& a, bool res, bool noise, cudaStream_t st) {
-    const int cpt = resident_cpt(a.geo.nx * a.geo.ny, sizeof(T) == 8, res);
+    const int cpt = resident_cpt((size_t)a.geo.nx * (size_t)a.geo.ny, sizeof(T) == 8, res);
     if (cpt == 0) return cudaErrorInvalidConfiguration;
 #define PHX_RES_CASE(R, NZ)                                                      \
     if (res == R && noise == NZ) {                                               \

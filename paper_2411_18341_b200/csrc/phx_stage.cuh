@@ -347,7 +347,7 @@ stage_kernel(const __grid_constant__ StageArgs<T> a) {
                     if (RES) nn[s][i] = cur[s].nacc[i] + w_dt * Kn;
                     if (NOISE) {
                         // dW of Eq. (22): variance sig2 (gamma_c + R n_t) per real component
-                        const uint32_t cell = (uint32_t)(j * g.nx + col.x0 + i);
+                        const uint32_t cell = (uint32_t)j * (uint32_t)g.nx + (uint32_t)(col.x0 + i);   // < 2^32 (desc_ok), unsigned product
                         const uint4 w = noise_words(a.seed, blockIdx.z, step, cell);
                         const C xi = s == 0 ? normal_pair(w.x, w.y, T(0)) : normal_pair(w.z, w.w, T(0));
                         const T nt = RES ? cur[s].n[i] : T(0);

@@ -10,6 +10,29 @@ def rel_l2(a, b):
 
 TOL = {"c32": 2e-5, "c64": 1e-12}   # BASELINE.json north_star: relative L2 after N steps
 
+# Element-wise guard next to every relative-L2 bar: max |got - ref| <= ELEM_C * tol * max |ref|.  The L2 norm averages
+# a localised error away (one wrong column of 4096 at relative size 1e-3 contributes 1.5e-5); rounding errors are spread
+# evenly, so their largest element stays within a few standard deviations of the rms error (5.5 sigma over 1e7 cells)
+# and rms |ref| <= max |ref|: a field inside the L2 bar is inside this one with ELEM_C = 8, a seam error is not.
+ELEM_C = 8.0
+
+
+def max_abs_ratio(a, b):
+    """max |a - b| / max |b| (the element-wise error in units of the largest reference element)."""
+    a = np.asarray(a, dtype=np.complex128 if np.iscomplexobj(a) else np.float64)
+    b = np.asarray(b, dtype=a.dtype)
+    return float(np.max(np.abs(a - b)) / max(float(np.max(np.abs(b))), 1e-300))
+
+
+def check_close(got, ref, tol, what):
+    """The two bars of every parity comparison: relative L2 <= tol and max |delta| <= ELEM_C tol max |ref|."""
+    assert np.all(np.isfinite(got)), f"{what}: non-finite values on the GPU"
+    err = rel_l2(got, ref)
+    assert err <= tol, f"{what}: rel L2 {err:.3e} > {tol:.1e}"
+    emax = max_abs_ratio(got, ref)
+    assert emax <= ELEM_C * tol, f"{what}: max |delta| / max |ref| = {emax:.3e} > {ELEM_C * tol:.1e}"
+    return err
+
 
 def make_oracle(w, bc=(0, 0), E=None, extra_params=None):
     import oracle as orc
@@ -47,13 +70,10 @@ def make_gpu(w, bc=(0, 0), E=None, extra_params=None, variant=0, tuning=None):
 
 
 def compare(g, o, w, tol=None):
-    """Element-wise comparison of every state field; returns dict field -> relative L2 error."""
+    """Element-wise comparison of every state field (relative L2 and largest element, check_close); returns dict
+    field -> relative L2 error."""
     tol = TOL[w.prec] if tol is None else tol
     errs = {}
     for name in w.fields:
-        got = g.read_field(name)
-        ref = getattr(o, name)
-        errs[name] = rel_l2(got, ref)
-        assert np.all(np.isfinite(got)), f"{name}: non-finite values on the GPU"
-        assert errs[name] <= tol, f"{w.name} {name}: rel L2 {errs[name]:.3e} > {tol:.1e}"
+        errs[name] = check_close(g.read_field(name), getattr(o, name), tol, f"{w.name} {name}")
     return errs

@@ -208,6 +208,9 @@ def test_device_buffers_and_api_errors():
     with pytest.raises(phx.PhxError) as e:
         g.set_field("n_p", np.zeros((1, w.ny, w.nx), np.float32))
     assert e.value.status == phx.PHX_ERR_UNSUPPORTED
+    with pytest.raises(phx.PhxError) as e:         # a pump needs a reservoir (Eq. (17))
+        g.set_potential_pump(None, np.ones((w.ny, w.nx), np.float32))
+    assert e.value.status == phx.PHX_ERR_UNSUPPORTED
     assert g.set_params(phx.make_params(dt=1.0)) == phx.PHX_WARN_UNSTABLE
     assert g.set_params(phx.make_params(**w.params)) == phx.PHX_OK
     dev_psi = torch.from_numpy(w.fields["psi_p"]).cuda()

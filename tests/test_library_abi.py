@@ -65,6 +65,13 @@ def test_invalid_descriptor_and_no_device_fail_loudly(libpath):
     ok = binding.phx_grid_desc(64, 64, 1, 0.5, 0.5, 0, 0, 0, 0, 0, None, 0, None)
     n = lib.phx_workspace_bytes(C.byref(ok))
     assert n >= 64 * 64 * 8 * 4
+    # plane sizes up to 2^32 - 1 cells are admitted (the noise counter holds the cell index in 32 bits); the sizes are
+    # computed in size_t: a 50 000^2 complex fp32 scalar grid needs 4 complex planes + V, P, E
+    big = binding.phx_grid_desc(50000, 50000, 1, 0.5, 0.5, 0, 0, 1, 0, 0, None, 0, None)
+    nb = lib.phx_workspace_bytes(C.byref(big))
+    assert nb >= 4 * 50000 * 50000 * 8 and nb < 8 * 50000 * 50000 * 8
+    too_big = binding.phx_grid_desc(70000, 70000, 1, 0.5, 0.5, 0, 0, 0, 0, 0, None, 0, None)
+    assert lib.phx_workspace_bytes(C.byref(too_big)) == 0
     import torch
     if not torch.cuda.is_available():
         h = C.c_void_p()

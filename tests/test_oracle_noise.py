@@ -134,3 +134,19 @@ def test_philox_matches_curand_header_on_random_inputs(tmp_path):
                            ref.ctypes.data_as(C.c_void_p), C.c_int64(n))
     got = np.array([orc.philox4x32_10(ctr[i], key[i]) for i in range(n)])
     assert np.array_equal(got, ref)
+
+
+def test_first_realisation_offsets_the_philox_key():
+    # element r of a batch == a batch of one with first_realisation = r (used to step single realisations of cfg5)
+    prm = orc.make_params(g=0.5, gamma_c=0.1, R=0.01, gamma_r=0.2, dt=0.02)
+    rng = np.random.default_rng(40)
+    a = rng.standard_normal((3, 6, 5)) + 1j * rng.standard_normal((3, 6, 5))
+    ob = orc.Oracle(5, 6, 0.5, 0.5, prm, model="reservoir", batch=3, noise=True, seed=9, P=np.ones((6, 5)))
+    ob.set_field("psi_p", a)
+    ob.step_rk4(4)
+    for r in range(3):
+        o1 = orc.Oracle(5, 6, 0.5, 0.5, prm, model="reservoir", batch=1, noise=True, seed=9, P=np.ones((6, 5)),
+                        first_realisation=r)
+        o1.set_field("psi_p", a[r:r + 1])
+        o1.step_rk4(4)
+        assert np.array_equal(o1.psi_p[0], ob.psi_p[r]) and np.array_equal(o1.n_p[0], ob.n_p[r])

@@ -78,6 +78,61 @@ def test_stencil_vs_fourier_symbol():
 
 
 # ----------------------------------------------------------------------------------------------
+# TE-TM operator J_pm = Delta_LT (d_x -+ i d_y)^2 on the other component, compact
+# nine-point form of DESIGN.md reading Q6, under periodic, zero and MIXED boundaries.
+# The reference is a dense matrix assembled from 1-D shift matrices by Kronecker products: a value
+# outside the grid along a zero axis is dropped, a periodic axis wraps.  (The 0-D plane-wave pin
+# below is periodic-only; this one fixes the corner rule of the mixed case.)
+# ----------------------------------------------------------------------------------------------
+def shift_1d(n, d, zero_bc):
+    """(S u)[i] = u[i + d] (d = +-1); outside the grid: 0 under a zero boundary, wrapped under a periodic one."""
+    S = np.zeros((n, n))
+    for i in range(n):
+        k = i + d
+        if 0 <= k < n:
+            S[i, k] = 1.0
+        elif not zero_bc:
+            S[i, k % n] = 1.0
+    return S
+
+
+def dense_operators(nx, ny, dx, dy, bc):
+    """d_xx, d_yy (three-point) and d_xy (product of the two central first differences) on the index k = j nx + i."""
+    Ix, Iy = np.eye(nx), np.eye(ny)
+    Xp, Xm = np.kron(Iy, shift_1d(nx, +1, bc[0])), np.kron(Iy, shift_1d(nx, -1, bc[0]))
+    Yp, Ym = np.kron(shift_1d(ny, +1, bc[1]), Ix), np.kron(shift_1d(ny, -1, bc[1]), Ix)
+    I = np.eye(nx * ny)
+    dxx = (Xp + Xm - 2 * I) / dx ** 2
+    dyy = (Yp + Ym - 2 * I) / dy ** 2
+    dxy = ((Xp - Xm) / (2 * dx)) @ ((Yp - Ym) / (2 * dy))
+    return dxx, dyy, dxy
+
+
+@pytest.mark.parametrize("nx,ny,dx,dy,bc", [(6, 5, 0.5, 0.5, (1, 1)), (7, 4, 0.3, 0.7, (1, 0)), (6, 5, 0.4, 0.9, (0, 1)),
+                                             (4, 7, 0.6, 0.35, (1, 0)), (3, 3, 0.5, 0.8, (0, 1)), (5, 6, 0.3, 0.45, (0, 0))])
+def test_tetm_operator_vs_dense_bruteforce(nx, ny, dx, dy, bc):
+    rng = np.random.default_rng(19)
+    a = rng.standard_normal((ny, nx)) + 1j * rng.standard_normal((ny, nx))
+    b = rng.standard_normal((ny, nx)) + 1j * rng.standard_normal((ny, nx))
+    hbar, m, beta = 0.8, 0.4, 0.13
+    o = orc.Oracle(nx, ny, dx, dy, orc.make_params(hbar=hbar, m=m, beta=beta, dt=0.1), model="spinor", bc=bc)
+    o.set_field("psi_p", a)
+    o.set_field("psi_m", b)
+    K = o.derivative()
+    dxx, dyy, dxy = dense_operators(nx, ny, dx, dy, bc)
+    lap = dxx + dyy
+    # Eq. (16): i hbar d_t psi_+- = -(hbar^2/2m) lap psi_+- + J_+- psi_-+,  J_+- = beta (d_x -+ i d_y)^2
+    Jp = beta * (dxx - dyy - 2j * dxy)          # (d_x - i d_y)^2 acts on psi_- in the psi_+ equation
+    Jm = beta * (dxx - dyy + 2j * dxy)
+    Kp = (-1j / hbar) * (-(hbar ** 2) / (2 * m) * (lap @ a.ravel()) + Jp @ b.ravel())
+    Km = (-1j / hbar) * (-(hbar ** 2) / (2 * m) * (lap @ b.ravel()) + Jm @ a.ravel())
+    assert rel_l2(K["K_p"].ravel(), Kp) < 1e-13
+    assert rel_l2(K["K_m"].ravel(), Km) < 1e-13
+    # the coupling alone (no kinetic term would hide a wrong corner: compare K minus the Laplacian part too)
+    assert rel_l2(K["K_p"].ravel() - 1j * hbar / (2 * m) * (lap @ a.ravel()), (-1j / hbar) * (Jp @ b.ravel())) < 1e-12
+
+
+# ----------------------------------------------------------------------------------------------
 # Linear scalar step: plane waves are exact eigenmodes, amplitude multiplies by R(z) per step
 # ----------------------------------------------------------------------------------------------
 @pytest.mark.parametrize("p,q", [(0, 0), (3, 0), (0, 5), (2, -3), (8, 8)])

@@ -50,6 +50,10 @@ def lib():
         _lib.orc_philox4x32_10.argtypes = [C.c_void_p] * 3
         _lib.orc_ensemble_mean_density.restype = None
         _lib.orc_ensemble_mean_density.argtypes = [C.c_int32] * 3 + [C.c_void_p] * 2
+        _lib.orc_dp54_tableau.restype = None
+        _lib.orc_dp54_tableau.argtypes = [C.c_int32] + [C.c_void_p] * 4
+        _lib.orc_step_dp54.restype = C.c_int32
+        _lib.orc_step_dp54.argtypes = [C.c_void_p] * 7 + [C.c_int32] + [C.c_void_p] * 4 + [C.c_int64, C.c_void_p]
     return _lib
 
 
@@ -71,6 +75,23 @@ def derive_coeffs(params: Params, dx: float, dy: float, prec32: bool) -> np.ndar
     out = np.zeros(NCOEF, dtype=np.float64)
     lib().orc_derive_coeffs(C.byref(params), dx, dy, int(bool(prec32)), _ptr(out))
     return out
+
+
+class Adaptive(C.Structure):
+    """Mirror of orc_adaptive (reading Q20)."""
+    _fields_ = [("atol", C.c_double), ("rtol", C.c_double), ("h_init", C.c_double), ("h_min", C.c_double),
+                ("h_max", C.c_double), ("t_end", C.c_double), ("max_attempts", C.c_int64)]
+
+
+class AdaptiveState(C.Structure):
+    _fields_ = [("t", C.c_double), ("h_next", C.c_double), ("n_accept", C.c_int64), ("n_reject", C.c_int64)]
+
+
+def dp54_tableau(prec32=False):
+    """(c[7], a[7][7], b[7], e[7]) of the Dormand-Prince 5(4) pair as the oracle uses them."""
+    c, a, b, e = np.zeros(7), np.zeros((7, 7)), np.zeros(7), np.zeros(7)
+    lib().orc_dp54_tableau(int(bool(prec32)), _ptr(c), _ptr(a), _ptr(b), _ptr(e))
+    return c, a, b, e
 
 
 class Oracle:
@@ -101,6 +122,22 @@ class Oracle:
         self.n_p = np.zeros(shape, np.float64) if self.reservoir else None
         self.n_m = np.zeros(shape, np.float64) if (self.reservoir and self.spinor) else None
         self.step = 0
+        self.prec32 = bool(prec32)
+        self.ad = AdaptiveState(0.0, 0.0, 0, 0)          # adaptive integrator: time, next step size, counters
+
+    def step_dp54(self, t_end, atol, rtol, h_init, h_min=1e-12, h_max=1e30, max_attempts=1 << 40, log_cap=1 << 16):
+        """Adaptive Dormand-Prince 5(4) from self.ad.t to t_end; returns the attempt log (accept, q, h, err)."""
+        ctl = Adaptive(atol, rtol, h_init, h_min, h_max, t_end, max_attempts)
+        acc, q = np.zeros(log_cap, np.int32), np.zeros(log_cap, np.int32)
+        h, err = np.zeros(log_cap), np.zeros(log_cap)
+        n = C.c_int64(0)
+        rc = lib().orc_step_dp54(C.byref(self.pb), _ptr(self.psi_p), _ptr(self.psi_m), _ptr(self.n_p), _ptr(self.n_m),
+                                 C.byref(ctl), C.byref(self.ad), int(self.prec32), _ptr(acc), _ptr(q), _ptr(h), _ptr(err),
+                                 log_cap, C.byref(n))
+        if rc != 0:
+            raise RuntimeError(f"orc_step_dp54: status {rc}")
+        k = min(n.value, log_cap)
+        return {"accept": acc[:k], "q": q[:k], "h": h[:k], "err": err[:k], "attempts": n.value}
 
     def set_field(self, name, arr):
         dst = getattr(self, name)

@@ -5,10 +5,15 @@
  * Written from /root/reference/PAPER.md; every function cites the passage it follows.
  * Deliberately unfused: K1..K4 and a stage buffer per field, full-grid loop per operation,
  * exactly the structure of Listing 1 and Fig. 2.
- * Build: g++ -O2 -ffp-contract=off (no fast-math, no OpenMP).
+ * Build: g++ -O2 -ffp-contract=off (no fast-math, no OpenMP): liboracle.so, the parity oracle, one thread.
+ * The "#pragma omp parallel for" lines over the rows / cells of each full-grid loop are ignored by that build; the
+ * SAME source compiled with -fopenmp (liboracle_omp.so, oracle/build.py) is the all-host-cores leg of bench.py's
+ * cpu_baseline and nothing else.  Every loop iteration writes its own cells only, so
+ * the threaded build computes the same bits.
  */
 #include "phx_oracle.h"
 
+#include <algorithm>
 #include <cmath>
 #include <complex>
 #include <cstddef>
@@ -65,6 +70,7 @@ void derivative(const orc_problem& pb, double t, const cplx* yp, const cplx* ym,
         double* Kn = s == 0 ? Knp : Knm;
         const double sign = s == 0 ? -1.0 : +1.0;  /* (d_x - i d_y)^2 in the psi_+ equation */
 
+#pragma omp parallel for schedule(static)
         for (int j = 0; j < pb.ny; ++j) {
             for (int i = 0; i < pb.nx; ++i) {
                 const size_t k = (size_t)j * pb.nx + i;
@@ -113,6 +119,7 @@ void derivative(const orc_problem& pb, double t, const cplx* yp, const cplx* ym,
 /* The paper's INTERMEDIATE_SUM_K (Eq. (9) :208): z = x + alpha*y. */
 template <class T>
 void two_term_sum(size_t n, const T* x, double alpha, const T* y, T* z) {
+#pragma omp parallel for schedule(static)
     for (size_t k = 0; k < n; ++k) z[k] = x[k] + alpha * y[k];
 }
 
@@ -120,6 +127,7 @@ void two_term_sum(size_t n, const T* x, double alpha, const T* y, T* z) {
 template <class T>
 void five_term_sum(size_t n, T* x, double a1, const T* y1, double a2, const T* y2, double a3, const T* y3,
                    double a4, const T* y4) {
+#pragma omp parallel for schedule(static)
     for (size_t k = 0; k < n; ++k) x[k] = x[k] + a1 * y1[k] + a2 * y2[k] + a3 * y3[k] + a4 * y4[k];
 }
 
@@ -268,6 +276,7 @@ int32_t orc_step_rk4(const orc_problem* pb, double* psi_p_, double* psi_m_, doub
             /* dW of Eq. (22): per real component variance sig2*(gamma_c + R n_t), n_t the reservoir
              * at the start of the step.  Words 0,1 drive psi_+, words 2,3 drive psi_-. */
             if (pb->noise) {
+#pragma omp parallel for schedule(static)
                 for (size_t k = 0; k < N; ++k) {
                     const uint32_t ctr[4] = {(uint32_t)k, (uint32_t)(step & 0xffffffffu), (uint32_t)(step >> 32), 0u};
                     const uint32_t key[2] = {pb->seed, pb->first_realisation + (uint32_t)r};
@@ -284,6 +293,165 @@ int32_t orc_step_rk4(const orc_problem* pb, double* psi_p_, double* psi_m_, doub
             }
         }
     }
+    return 0;
+}
+
+/* Dormand-Prince 5(4) tableau (J. Comput. Appl. Math. 6 (1980) 19, Table 2), as quotients. */
+void orc_dp54_tableau(int32_t prec32, double* c, double* a, double* b, double* e) {
+    const double C[7] = {0.0, 1.0 / 5.0, 3.0 / 10.0, 4.0 / 5.0, 8.0 / 9.0, 1.0, 1.0};
+    const double A[7][7] = {
+        {0, 0, 0, 0, 0, 0, 0},
+        {1.0 / 5.0, 0, 0, 0, 0, 0, 0},
+        {3.0 / 40.0, 9.0 / 40.0, 0, 0, 0, 0, 0},
+        {44.0 / 45.0, -56.0 / 15.0, 32.0 / 9.0, 0, 0, 0, 0},
+        {19372.0 / 6561.0, -25360.0 / 2187.0, 64448.0 / 6561.0, -212.0 / 729.0, 0, 0, 0},
+        {9017.0 / 3168.0, -355.0 / 33.0, 46732.0 / 5247.0, 49.0 / 176.0, -5103.0 / 18656.0, 0, 0},
+        {35.0 / 384.0, 0.0, 500.0 / 1113.0, 125.0 / 192.0, -2187.0 / 6784.0, 11.0 / 84.0, 0}};
+    /* embedded fourth-order weights b* */
+    const double BS[7] = {5179.0 / 57600.0, 0.0, 7571.0 / 16695.0, 393.0 / 640.0, -92097.0 / 339200.0,
+                          187.0 / 2100.0, 1.0 / 40.0};
+    for (int s = 0; s < 7; ++s) {
+        c[s] = round_to(C[s], prec32);
+        for (int j = 0; j < 7; ++j) a[7 * s + j] = round_to(A[s][j], prec32);
+        b[s] = round_to(A[6][s], prec32);
+        e[s] = round_to(A[6][s] - BS[s], prec32);
+    }
+}
+
+int32_t orc_step_dp54(const orc_problem* pb, double* psi_p_, double* psi_m_, double* n_p_, double* n_m_,
+                      const orc_adaptive* ctl, orc_adaptive_state* st, int32_t prec32,
+                      int32_t* log_accept, int32_t* log_q, double* log_h, double* log_err,
+                      int64_t log_cap, int64_t* n_log) {
+    if (!pb || !psi_p_ || !ctl || !st || pb->nx < 1 || pb->ny < 1 || pb->batch < 1) return 1;
+    if (pb->spinor && !psi_m_) return 1;
+    if (pb->reservoir && (!n_p_ || (pb->spinor && !n_m_))) return 1;
+    if (!(ctl->atol >= 0) || !(ctl->rtol >= 0) || !(ctl->atol + ctl->rtol > 0) || !(ctl->h_min > 0) ||
+        !(ctl->h_max >= ctl->h_min))
+        return 1;
+    if (pb->noise) return 2;
+
+    const size_t N = (size_t)pb->nx * pb->ny;
+    const int ncomp = pb->spinor ? 2 : 1;
+    const bool res = pb->reservoir != 0;
+    const int B = pb->batch;
+    double c[7], a[49], b[7], e[7];
+    orc_dp54_tableau(prec32, c, a, b, e);
+
+    /* per batch element and field: K_1..K_7, the stage input Y and the candidate u_new */
+    std::vector<cplx> K[7][2], Y[2], Un[2];
+    std::vector<double> Kn[7][2], Yn[2], Unn[2];
+    for (int s = 0; s < ncomp; ++s) {
+        Y[s].resize(N * B);
+        Un[s].resize(N * B);
+        for (int q = 0; q < 7; ++q) K[q][s].resize(N * B);
+        if (res) {
+            Yn[s].resize(N * B);
+            Unn[s].resize(N * B);
+            for (int q = 0; q < 7; ++q) Kn[q][s].resize(N * B);
+        }
+    }
+    cplx* psi[2] = {(cplx*)psi_p_, pb->spinor ? (cplx*)psi_m_ : nullptr};
+    double* nn[2] = {res ? n_p_ : nullptr, (res && pb->spinor) ? n_m_ : nullptr};
+
+    /* f on every batch element */
+    auto f_all = [&](double t, cplx* const y[2], double* const yn[2], int q) {
+        for (int r = 0; r < B; ++r) {
+            const size_t o = (size_t)r * N;
+            derivative(*pb, t, y[0] + o, y[1] ? y[1] + o : nullptr, yn[0] ? yn[0] + o : nullptr,
+                       yn[1] ? yn[1] + o : nullptr, K[q][0].data() + o, ncomp == 2 ? K[q][1].data() + o : nullptr,
+                       res ? Kn[q][0].data() + o : nullptr, (res && ncomp == 2) ? Kn[q][1].data() + o : nullptr);
+        }
+    };
+
+    double t = st->t;
+    double h = st->h_next > 0 ? st->h_next : ctl->h_init;
+    if (h < ctl->h_min) h = ctl->h_min;
+    if (h > ctl->h_max) h = ctl->h_max;
+    bool have_k1 = false;                 /* FSAL: K_1 of this attempt is K_7 of the last accepted one */
+    int64_t attempts = 0;
+    while (t < ctl->t_end && attempts < ctl->max_attempts) {
+        /* the step actually taken: clipped so that the call lands on t_end; rounded once to T */
+        const bool clipped = t + h >= ctl->t_end;
+        const double hu = round_to(clipped ? ctl->t_end - t : h, prec32);
+
+        if (!have_k1) {
+            f_all(t, psi, nn, 0);
+            have_k1 = true;
+        }
+        /* stages 2..7: Y_s = u + hu sum_j a_sj K_j, K_s = f(Y_s, t + c_s hu); Y_7 is u_new */
+        for (int s = 1; s < 7; ++s) {
+            for (int comp = 0; comp < ncomp; ++comp) {
+                cplx* dst = s == 6 ? Un[comp].data() : Y[comp].data();
+                for (size_t k = 0; k < N * B; ++k) {
+                    cplx acc(0.0, 0.0);
+                    for (int j = 0; j < s; ++j) acc += a[7 * s + j] * K[j][comp][k];
+                    dst[k] = psi[comp][k] + hu * acc;
+                }
+                if (res) {
+                    double* dn = s == 6 ? Unn[comp].data() : Yn[comp].data();
+                    for (size_t k = 0; k < N * B; ++k) {
+                        double acc = 0.0;
+                        for (int j = 0; j < s; ++j) acc += a[7 * s + j] * Kn[j][comp][k];
+                        dn[k] = nn[comp][k] + hu * acc;
+                    }
+                }
+            }
+            cplx* const ys[2] = {s == 6 ? Un[0].data() : Y[0].data(),
+                                 ncomp == 2 ? (s == 6 ? Un[1].data() : Y[1].data()) : nullptr};
+            double* const yns[2] = {res ? (s == 6 ? Unn[0].data() : Yn[0].data()) : nullptr,
+                                    (res && ncomp == 2) ? (s == 6 ? Unn[1].data() : Yn[1].data()) : nullptr};
+            f_all(t + c[s] * hu, ys, yns, s);
+        }
+        /* error norm */
+        double err = 0.0;
+        for (int comp = 0; comp < ncomp; ++comp) {
+            for (size_t k = 0; k < N * B; ++k) {
+                cplx E(0.0, 0.0);
+                for (int j = 0; j < 7; ++j) E += e[j] * K[j][comp][k];
+                const double sc = ctl->atol + ctl->rtol * std::max(std::abs(psi[comp][k]), std::abs(Un[comp][k]));
+                err = std::max(err, std::abs(hu * E) / sc);
+            }
+            if (res)
+                for (size_t k = 0; k < N * B; ++k) {
+                    double E = 0.0;
+                    for (int j = 0; j < 7; ++j) E += e[j] * Kn[j][comp][k];
+                    const double sc = ctl->atol + ctl->rtol * std::max(std::fabs(nn[comp][k]), std::fabs(Unn[comp][k]));
+                    err = std::max(err, std::fabs(hu * E) / sc);
+                }
+        }
+        /* controller */
+        const bool accept = err <= 1.0 || h <= ctl->h_min;       /* a proposal that cannot shrink is taken as it is */
+        double fac = err > 0.0 ? 0.9 * std::pow(err, -0.2) : 4.0;
+        fac = std::min(4.0, std::max(0.25, fac));
+        const int32_t q = (int32_t)std::floor(16.0 * fac);
+        if (attempts < log_cap) {
+            if (log_accept) log_accept[attempts] = accept ? 1 : 0;
+            if (log_q) log_q[attempts] = q;
+            if (log_h) log_h[attempts] = hu;
+            if (log_err) log_err[attempts] = err;
+        }
+        ++attempts;
+        if (accept) {
+            for (int comp = 0; comp < ncomp; ++comp) {
+                std::memcpy(psi[comp], Un[comp].data(), N * B * sizeof(cplx));
+                K[0][comp].swap(K[6][comp]);                      /* FSAL */
+                if (res) {
+                    std::memcpy(nn[comp], Unn[comp].data(), N * B * sizeof(double));
+                    Kn[0][comp].swap(Kn[6][comp]);
+                }
+            }
+            t = clipped ? ctl->t_end : t + hu;
+            ++st->n_accept;
+            /* (a clipped step says nothing about the step size the dynamics allow: the proposal h is kept) */
+            if (!clipped) h = std::min(ctl->h_max, std::max(ctl->h_min, hu * (double)q / 16.0));
+        } else {
+            ++st->n_reject;
+            h = std::min(ctl->h_max, std::max(ctl->h_min, hu * (double)q / 16.0));
+        }
+    }
+    st->t = t;
+    st->h_next = h;
+    if (n_log) *n_log = attempts;
     return 0;
 }
 

@@ -15,6 +15,8 @@
  * All arithmetic is IEEE double, one thread, no FMA contraction, no blocking or fusion.
  * The readings taken where the paper is silent or garbled are listed in DESIGN.md section 3.
  *
+ * Adaptive Dormand-Prince 5(4): orc_step_dp54 below (the paper names the method only).
+ *
  * Pins (tests/test_oracle_*.py, all -m "not gpu"): stencil vs. dense brute force and vs. its
  * Fourier symbol; plane-wave amplification R(z)^N; loss and norm closed forms; reduction of
  * plane-wave states to a 0-dimensional RK4 written independently in Python (nonlinearity,
@@ -85,6 +87,49 @@ void orc_derivative(const orc_problem* pb, double t,
  * (keys the noise and fixes t = step0*dt for the drive).  Returns 0, or 1 on bad arguments. */
 int32_t orc_step_rk4(const orc_problem* pb, double* psi_p, double* psi_m, double* n_p, double* n_m,
                      uint64_t step0, int64_t n_steps);
+
+/* ---- adaptive Dormand-Prince 5(4) --------------------------------------------
+ * The paper only NAMES the method ("higher-order methods like the RK-Fehlberg or Dormand-Prince can be
+ * used for systems requiring adaptive time-stepping"; "adaptive Runge-Kutta methods ... could be
+ * optimized within the framework of PHOENIX").  Everything below is DESIGN.md reading Q20:
+ *   - tableau: Dormand & Prince, J. Comput. Appl. Math. 6 (1980) 19, the seven-stage 5(4) pair with FSAL,
+ *     written out in orc_dp54_tableau; each coefficient is evaluated as a double quotient and, with prec32,
+ *     rounded once to float;
+ *   - stage s: Y_s = u + h sum_j a_sj K_j, K_s = f(Y_s, t + c_s h); u_new = Y_7 (fifth order);
+ *     error estimate E = h sum_j e_j K_j with e = b - b* (b* the embedded fourth-order weights);
+ *   - error norm: err = max over all cells, components, reservoirs and batch elements of
+ *     |E| / (atol + rtol max(|u|, |u_new|))  (complex modulus for psi, absolute value for n);
+ *   - accept iff err <= 1 (or the proposed step is already h_min); step factor q/16 with
+ *     q = floor(16 min(4, max(1/4, 0.9 err^(-1/5)))) (q = 64 for err = 0): the QUANTISED factor makes the
+ *     step-size sequence an integer sequence that the CUDA path must reproduce bit for bit;
+ *     h <- clamp(h_used q/16, h_min, h_max) after every attempt, accepted or not;
+ *   - a step that would pass t_end is clipped to land on it exactly; after an accepted clipped step the
+ *     unclipped proposal is kept for the next call; the step used is rounded once to float when prec32;
+ *   - one step size for the whole batch; noise is not supported (returns 2).
+ * Log: one record per ATTEMPT (accepted or rejected): accept flag, q, h used, err. */
+typedef struct {
+    double atol, rtol;           /* error norm */
+    double h_init;               /* first step size tried (used when state->h_next <= 0) */
+    double h_min, h_max;         /* clamp of the step size */
+    double t_end;                /* integrate until t == t_end */
+    int64_t max_attempts;        /* stop after this many attempts of this call even if t < t_end */
+} orc_adaptive;
+
+typedef struct {
+    double t;                    /* current time (in/out) */
+    double h_next;               /* step size the next attempt will try (in/out; <= 0: use h_init) */
+    int64_t n_accept, n_reject;  /* counters (in/out) */
+} orc_adaptive_state;
+
+/* c[7], a[7][7] (row s, column j < s), b[7] (= a[6][.]), e[7] = b - b*. */
+void orc_dp54_tableau(int32_t prec32, double* c, double* a, double* b, double* e);
+
+/* Integrates from st->t to ctl->t_end.  log_* may be NULL; at most log_cap records are written, the
+ * number of attempts made is returned in *n_log.  Returns 0; 1 on bad arguments; 2 if noise is on. */
+int32_t orc_step_dp54(const orc_problem* pb, double* psi_p, double* psi_m, double* n_p, double* n_m,
+                      const orc_adaptive* ctl, orc_adaptive_state* st, int32_t prec32,
+                      int32_t* log_accept, int32_t* log_q, double* log_h, double* log_err,
+                      int64_t log_cap, int64_t* n_log);
 
 /* Philox4x32-10 (Salmon et al., SC'11): one block. */
 void orc_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]);

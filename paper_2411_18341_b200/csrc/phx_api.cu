@@ -87,6 +87,7 @@ struct phx_grid {
     int rows, vec, graph_steps, gsteps;
     int parity;             // variant STEP ping-pongs the state: 0 = state in psi/n, 1 = state in ya/na
     int step_ly, step_vec;  // variant STEP geometry (0 = automatic)
+    int step_bulk;          // variant STEP fetch path: -1 automatic, 0 register loads, 1 bulk copies into a shared-memory ring
     int async_host;         // 1: host copies of set_field / read_field do not synchronise (pinned buffers, caller syncs)
     cudaGraphExec_t g1[2], gN;  // one step from parity 0 / 1; graph_steps steps from parity 0
     bool graphs_valid;
@@ -166,7 +167,9 @@ void fill_geo_coef(const phx_grid* g, Geom& geo, Coef<T>& k) {
     k.hgc = (T)c[7]; k.gamr = (T)c[8]; k.bxx = (T)c[9]; k.byy = (T)c[10]; k.bxy = (T)c[11]; k.dt = (T)c[12];
     k.hdt = (T)(0.5 * c[12]);           // exact
     k.dt6 = (T)c[13]; k.dt3 = (T)c[14]; k.sig2 = (T)c[15]; k.doff = (T)c[16];
-    k.r13 = (T)(c[13] / (0.5 * c[12]));
+    const double r13 = c[13] / (0.5 * c[12]);
+    k.r13 = (T)r13;
+    k.r13lo = (T)(r13 - (double)k.r13);
     k.omega = c[17];
     k.dt_d = c[12];
 }
@@ -247,21 +250,29 @@ int step_vec(const phx_grid* g) {
 // dx == dy: the isotropic form of the Laplacian (cx == cy bit for bit, both derived from the same expression)
 bool step_iso(const phx_grid* g) { return g->d.dx == g->d.dy; }
 
+// The bulk-copy fetch path (phx_step.cuh, BULK): periodic boundaries, rows whose pieces are 16-byte aligned and sized.
+bool step_bulk(const phx_grid* g) {
+    if (g->d.bc_x || g->d.bc_y) return false;
+    if (((size_t)g->d.nx * real_bytes(g)) % 16 != 0) return false;
+    if (g->d.nx < 32 * step_vec(g)) return false;       // a strip wraps at most once
+    return g->step_bulk == 1;                           // opt-in: measured slower than the register loads
+}
+
 int step_occupancy(const phx_grid* g, int vec) {
-    const bool noise = g->d.noise != 0, zbc = g->d.bc_x || g->d.bc_y, iso = step_iso(g), drive = g->hasE;
+    const bool noise = g->d.noise != 0, zbc = g->d.bc_x || g->d.bc_y, iso = step_iso(g), drive = g->hasE, bulk = step_bulk(g);
     if (g->d.prec == PHX_C32) {
         switch (g->d.model) {
-            case 0: return occupancy_step_32_0(noise, zbc, iso, drive, vec);
-            case 1: return occupancy_step_32_1(noise, zbc, iso, drive, vec);
-            case 2: return occupancy_step_32_2(noise, zbc, iso, drive, vec);
-            default: return occupancy_step_32_3(noise, zbc, iso, drive, vec);
+            case 0: return occupancy_step_32_0(noise, zbc, iso, drive, bulk, vec);
+            case 1: return occupancy_step_32_1(noise, zbc, iso, drive, bulk, vec);
+            case 2: return occupancy_step_32_2(noise, zbc, iso, drive, bulk, vec);
+            default: return occupancy_step_32_3(noise, zbc, iso, drive, bulk, vec);
         }
     }
     switch (g->d.model) {
-        case 0: return occupancy_step_64_0(noise, zbc, iso, drive, vec);
-        case 1: return occupancy_step_64_1(noise, zbc, iso, drive, vec);
-        case 2: return occupancy_step_64_2(noise, zbc, iso, drive, vec);
-        default: return occupancy_step_64_3(noise, zbc, iso, drive, vec);
+        case 0: return occupancy_step_64_0(noise, zbc, iso, drive, bulk, vec);
+        case 1: return occupancy_step_64_1(noise, zbc, iso, drive, bulk, vec);
+        case 2: return occupancy_step_64_2(noise, zbc, iso, drive, bulk, vec);
+        default: return occupancy_step_64_3(noise, zbc, iso, drive, bulk, vec);
     }
 }
 
@@ -344,20 +355,20 @@ cudaError_t enqueue_step_fused(phx_grid* g, cudaStream_t st, int parity) {
     a.ly = step_rows_per_chunk(g, vec);
     const dim3 grid((a.strips + PHX_STEP_WARPS - 1) / PHX_STEP_WARPS, (g->d.ny + a.ly - 1) / a.ly, g->d.batch);
     if (grid.y > 65535u) return cudaErrorInvalidConfiguration;
-    const bool noise = g->d.noise != 0, zbc = g->d.bc_x || g->d.bc_y, iso = step_iso(g);
+    const bool noise = g->d.noise != 0, zbc = g->d.bc_x || g->d.bc_y, iso = step_iso(g), bulk = step_bulk(g);
     if constexpr (sizeof(T) == 4) {
         switch (g->d.model) {
-            case 0: return launch_step_32_0(a, noise, zbc, iso, vec, grid, st);
-            case 1: return launch_step_32_1(a, noise, zbc, iso, vec, grid, st);
-            case 2: return launch_step_32_2(a, noise, zbc, iso, vec, grid, st);
-            default: return launch_step_32_3(a, noise, zbc, iso, vec, grid, st);
+            case 0: return launch_step_32_0(a, noise, zbc, iso, bulk, vec, grid, st);
+            case 1: return launch_step_32_1(a, noise, zbc, iso, bulk, vec, grid, st);
+            case 2: return launch_step_32_2(a, noise, zbc, iso, bulk, vec, grid, st);
+            default: return launch_step_32_3(a, noise, zbc, iso, bulk, vec, grid, st);
         }
     } else {
         switch (g->d.model) {
-            case 0: return launch_step_64_0(a, noise, zbc, iso, vec, grid, st);
-            case 1: return launch_step_64_1(a, noise, zbc, iso, vec, grid, st);
-            case 2: return launch_step_64_2(a, noise, zbc, iso, vec, grid, st);
-            default: return launch_step_64_3(a, noise, zbc, iso, vec, grid, st);
+            case 0: return launch_step_64_0(a, noise, zbc, iso, bulk, vec, grid, st);
+            case 1: return launch_step_64_1(a, noise, zbc, iso, bulk, vec, grid, st);
+            case 2: return launch_step_64_2(a, noise, zbc, iso, bulk, vec, grid, st);
+            default: return launch_step_64_3(a, noise, zbc, iso, bulk, vec, grid, st);
         }
     }
 }
@@ -522,6 +533,7 @@ phx_status phx_create_grid(phx_grid** out, const phx_grid_desc* desc) {
     g->graphs_valid = false;
     g->parity = 0;
     g->step_ly = g->step_vec = 0;
+    g->step_bulk = -1;
     g->async_host = 0;
     g->n_sm = prop.multiProcessorCount;
     g->l2_bytes = (size_t)prop.l2CacheSize;
@@ -763,6 +775,9 @@ phx_status phx_set_tuning(phx_grid* g, const char* key, int32_t value) {
         if (value == 4 && (g->d.model != PHX_SCALAR || g->d.prec != PHX_C32)) return fail(g, PHX_ERR_UNSUPPORTED, "step_vec=4 exists for the scalar fp32 model only");
         if (value == 2 && g->d.prec == PHX_C64 && g->d.model != PHX_SCALAR) return fail(g, PHX_ERR_UNSUPPORTED, "step_vec=2 in fp64 exists for the scalar model only");
         g->step_vec = value;
+    } else if (!std::strcmp(key, "step_bulk")) {      // variant STEP fetch path: -1 automatic, 0 register loads, 1 bulk copies
+        if (value < -1 || value > 1) return PHX_ERR_INVALID_ARG;
+        g->step_bulk = value;
     } else if (!std::strcmp(key, "async_host_copies")) {   // 1: phx_set_field / phx_read_field with PHX_HOST do not synchronise
         if (value != 0 && value != 1) return PHX_ERR_INVALID_ARG;
         g->async_host = value;

@@ -20,7 +20,9 @@ template <typename T> __device__ __forceinline__ typename Cx<T>::type mk(T re, T
 template <typename T>
 struct Coef {
     T cx, cy, ih, g, gx, gr, Rr, hgc, gamr, bxx, byy, bxy, dt, hdt, dt6, dt3, sig2, doff;
-    T r13;          // dt6 / hdt, used to rebuild dt6*K1 from y2 - psi (variant STAGE)
+    T r13, r13lo;   // dt6 / hdt as an unevaluated sum of two T (hi + lo), used to rebuild dt6*K1 from y2 - psi (variant STAGE,
+                    // DESIGN.md section 5.1): with one T the weight of K1 differs from the canonical dt6 by a relative 2^-25,
+                    // a systematic error that grows linearly with the step count (3e-5 after 10^4 fp32 steps)
     double omega;   // drive frequency, phase evaluated in double
     double dt_d;    // dt as double (the T-rounded value widened), for t = step*dt
 };

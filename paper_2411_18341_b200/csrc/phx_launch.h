@@ -14,6 +14,10 @@
 #define PHX_STEP_LEAD 1
 #endif
 #define PHX_STEP_RING (4 + PHX_STEP_LEAD)
+// Bulk-copy fetch path of variant STEP: stages of the per-warp shared-memory ring (rows in flight = DEPTH - 1); power of 2.
+#ifndef PHX_STEP_DEPTH
+#define PHX_STEP_DEPTH 8
+#endif
 
 namespace phx {
 
@@ -31,14 +35,14 @@ PHX_DECL_STAGE(64, double)
 template <typename T> struct StepArgs;
 
 #define PHX_DECL_STEP(P, T)                                                                                      \
-    cudaError_t launch_step_##P##_0(const StepArgs<T>&, bool noise, bool zbc, bool iso, int vec, dim3 grid, cudaStream_t); \
-    cudaError_t launch_step_##P##_1(const StepArgs<T>&, bool noise, bool zbc, bool iso, int vec, dim3 grid, cudaStream_t); \
-    cudaError_t launch_step_##P##_2(const StepArgs<T>&, bool noise, bool zbc, bool iso, int vec, dim3 grid, cudaStream_t); \
-    cudaError_t launch_step_##P##_3(const StepArgs<T>&, bool noise, bool zbc, bool iso, int vec, dim3 grid, cudaStream_t); \
-    int occupancy_step_##P##_0(bool noise, bool zbc, bool iso, bool drive, int vec);                                          \
-    int occupancy_step_##P##_1(bool noise, bool zbc, bool iso, bool drive, int vec);                                          \
-    int occupancy_step_##P##_2(bool noise, bool zbc, bool iso, bool drive, int vec);                                          \
-    int occupancy_step_##P##_3(bool noise, bool zbc, bool iso, bool drive, int vec);
+    cudaError_t launch_step_##P##_0(const StepArgs<T>&, bool noise, bool zbc, bool iso, bool bulk, int vec, dim3 grid, cudaStream_t); \
+    cudaError_t launch_step_##P##_1(const StepArgs<T>&, bool noise, bool zbc, bool iso, bool bulk, int vec, dim3 grid, cudaStream_t); \
+    cudaError_t launch_step_##P##_2(const StepArgs<T>&, bool noise, bool zbc, bool iso, bool bulk, int vec, dim3 grid, cudaStream_t); \
+    cudaError_t launch_step_##P##_3(const StepArgs<T>&, bool noise, bool zbc, bool iso, bool bulk, int vec, dim3 grid, cudaStream_t); \
+    int occupancy_step_##P##_0(bool noise, bool zbc, bool iso, bool drive, bool bulk, int vec);                                          \
+    int occupancy_step_##P##_1(bool noise, bool zbc, bool iso, bool drive, bool bulk, int vec);                                          \
+    int occupancy_step_##P##_2(bool noise, bool zbc, bool iso, bool drive, bool bulk, int vec);                                          \
+    int occupancy_step_##P##_3(bool noise, bool zbc, bool iso, bool drive, bool bulk, int vec);
 PHX_DECL_STEP(32, float)
 PHX_DECL_STEP(64, double)
 #undef PHX_DECL_STEP

@@ -99,7 +99,7 @@ resident_kernel(const __grid_constant__ ResidentArgs<T> a) {
                     if (NOISE) {
                         const uint4 wd = noise_words(a.seed, blockIdx.x, step, (uint32_t)c);
                         const T nt = RES ? nn[q] : T(0);          // reservoir at the start of the step
-                        nw = add2(nw, noise_increment(wd.x, wd.y, k.sig2 * (T(2) * k.hgc + k.Rr * nt)));
+                        nw = add2(nw, noise_increment_sfu(wd.x, wd.y, k.sig2 * (T(2) * k.hgc + k.Rr * nt)));
                     }
                     psi[q] = nw;
                     if (RES) nn[q] = nacc[q] + w_dt * Kn;

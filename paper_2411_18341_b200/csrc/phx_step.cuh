@@ -93,6 +93,66 @@ template <int VEC> __device__ __forceinline__ void str(double* p, const double (
     else *p = v[0];
 }
 
+// ---- bulk-copy fetch path (template switch BULK): rows are brought from global memory into a per-warp ring of shared-memory
+// stages by 1-D bulk copies of the TMA unit (cp.async.bulk, one elected lane, completion on an mbarrier), DEPTH rows ahead
+// of their use, and read from there with 128-bit shared loads.  No register is tied up by a row in flight from DRAM. ----
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
+}
+// (the issuing instructions are predicated on `lead` -- one elected lane -- instead of sitting in a divergent branch)
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes, uint32_t lead) {
+    asm volatile("{\n.reg .pred p;\nsetp.ne.u32 p, %2, 0;\n@p mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n}"
+                 ::"r"(bar), "r"(bytes), "r"(lead) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred P1;\n"
+        "LAB_WAIT:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n"
+        "@P1 bra DONE;\n"
+        "bra LAB_WAIT;\n"
+        "DONE:\n"
+        "}" ::"r"(bar), "r"(parity) : "memory");
+}
+// non-blocking: has the phase with this parity completed?
+__device__ __forceinline__ uint32_t mbar_test(uint32_t bar, uint32_t parity) {
+    uint32_t ok;
+    asm volatile("{\n.reg .pred p;\nmbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\nselp.u32 %0, 1, 0, p;\n}"
+                 : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+    return ok;
+}
+// global -> shared bulk copy of `bytes` (a multiple of 16; both addresses 16-byte aligned), completing on `bar`
+__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar, uint32_t lead) {
+    asm volatile("{\n.reg .pred p;\nsetp.ne.u32 p, %4, 0;\n"
+                 "@p cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];\n}"
+                 ::"r"(dst), "l"(src), "r"(bytes), "r"(bar), "r"(lead) : "memory");
+}
+template <int VEC> __device__ __forceinline__ void ldsc(const float2* p, float2 (&v)[VEC]) {
+    if constexpr (VEC % 2 == 0) {
+#pragma unroll
+        for (int h = 0; h < VEC / 2; ++h) {
+            const float4 q = reinterpret_cast<const float4*>(p)[h];
+            v[2 * h] = make_float2(q.x, q.y);
+            v[2 * h + 1] = make_float2(q.z, q.w);
+        }
+    } else v[0] = *p;
+}
+template <int VEC> __device__ __forceinline__ void ldsc(const double2* p, double2 (&v)[VEC]) {
+#pragma unroll
+    for (int i = 0; i < VEC; ++i) v[i] = p[i];
+}
+template <int VEC> __device__ __forceinline__ void ldsr(const float* p, float (&v)[VEC]) {
+    if constexpr (VEC == 4) { const float4 q = *reinterpret_cast<const float4*>(p); v[0] = q.x; v[1] = q.y; v[2] = q.z; v[3] = q.w; }
+    else if constexpr (VEC == 2) { const float2 q = *reinterpret_cast<const float2*>(p); v[0] = q.x; v[1] = q.y; }
+    else v[0] = *p;
+}
+template <int VEC> __device__ __forceinline__ void ldsr(const double* p, double (&v)[VEC]) {
+    if constexpr (VEC == 2) { const double2 q = *reinterpret_cast<const double2*>(p); v[0] = q.x; v[1] = q.y; }
+    else v[0] = *p;
+}
+
 // DRAM -> L2 prefetch of the line holding p (no register is tied up; the register fetch one row ahead then hits L2).
 __device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
 
@@ -137,9 +197,29 @@ __device__ __forceinline__ void gather(const typename Cx<T>::type (&rs)[VEC], co
 // register either).  RING = 4 + LEAD is the longest life: psi rows j-2 .. j+1+LEAD and V rows j-3 .. j+LEAD, where LEAD
 // (PHX_STEP_LEAD, phx_launch.h) is the number of row iterations a fetch leads its first use by.
 
+// Byte layout of the per-warp shared-memory ring of the bulk-copy fetch path: PHX_STEP_DEPTH stages, each holding what one
+// row iteration fetches for the warp's strip of W columns: psi row j+1+LEAD of every component, then the row-local inputs
+// (n, V, P, E) of row j+LEAD.  Every offset is a multiple of 16 bytes (W * sizeof(T) >= 128).
+template <typename T, int VEC, int MODEL, bool DRIVE>
+struct StepSmem {
+    using C = typename Cx<T>::type;
+    static constexpr uint32_t NC = model_spinor(MODEL) ? 2 : 1;
+    static constexpr bool RES = model_reservoir(MODEL);
+    static constexpr uint32_t W = 32 * VEC;
+    static constexpr uint32_t PSI = 0;
+    static constexpr uint32_t N = PSI + NC * W * sizeof(C);
+    static constexpr uint32_t V = N + (RES ? NC * W * sizeof(T) : 0);
+    static constexpr uint32_t P = V + W * sizeof(T);
+    static constexpr uint32_t E = P + (RES ? W * sizeof(T) : 0);
+    static constexpr uint32_t STAGE = E + (DRIVE ? W * sizeof(C) : 0);
+    static constexpr uint32_t BARS = PHX_STEP_WARPS * PHX_STEP_DEPTH * 8;          // mbarriers, at the start
+    static constexpr uint32_t CTA = BARS + PHX_STEP_WARPS * PHX_STEP_DEPTH * STAGE;
+};
+
 // MINW: resident warps per SM the register budget is sized for.  ISO: dx == dy (scalar and reservoir models only).
 // DRIVE: coherent drive E(r) exp(-i omega t) (reading Q17), shared by both components.
-template <typename T, int VEC, int MODEL, bool NOISE, bool ZBC, bool ISO, bool DRIVE, int MINW>
+// BULK: rows are fetched by TMA bulk copies into a shared-memory ring instead of register loads (periodic boundaries only).
+template <typename T, int VEC, int MODEL, bool NOISE, bool ZBC, bool ISO, bool DRIVE, int MINW, bool BULK>
 __global__ void __launch_bounds__(32 * PHX_STEP_WARPS, MINW / PHX_STEP_WARPS)
 step_kernel(const __grid_constant__ StepArgs<T> a) {
     using namespace stepk;
@@ -149,6 +229,7 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
     constexpr int NC = SPINOR ? 2 : 1;
     constexpr int W = 32 * VEC, OUTW = W - 8;
     constexpr int RING = PHX_STEP_RING, LEAD = PHX_STEP_LEAD;
+    static_assert(!(BULK && ZBC), "the bulk-copy fetch path is built for periodic boundaries");
     const Geom& g = a.geo;
     const Coef<T>& k = a.k;
     const int nx = g.nx, ny = g.ny;
@@ -293,6 +374,69 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
         if (!zy && qw == ny) { qw = 0; ew -= plane; }
     }
 
+    // ---- bulk-copy fetch path: the ring, its mbarriers and the issuer's state ------------------------------------------------
+    using SM = StepSmem<T, VEC, MODEL, DRIVE>;
+    constexpr int DEPTH = PHX_STEP_DEPTH;
+    extern __shared__ __align__(128) unsigned char step_smem[];
+    uint32_t bar0 = 0, ring0 = 0;                       // shared-window addresses of this warp's mbarriers and stages
+    const unsigned char* ringp = nullptr;
+    int fi = 0, fc = 0, ntot = 0;                       // next fetch to issue / to consume; fetches in all (= row iterations)
+    int qi = qw, qip = qw;                              // wrapped row of the psi / of the row-local inputs of fetch fi
+    uint32_t txbytes = 0;
+    int c0 = 0;                                         // wrapped first column of the strip
+    if constexpr (BULK) {
+        const int warp = threadIdx.x >> 5;
+        bar0 = smem_u32(step_smem) + warp * DEPTH * 8;
+        ringp = step_smem + SM::BARS + warp * DEPTH * SM::STAGE;
+        ring0 = smem_u32(ringp);
+        if (lane == 0) {
+#pragma unroll
+            for (int d = 0; d < DEPTH; ++d) mbar_init(bar0 + d * 8, 1);
+            asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        }
+        __syncwarp();
+        ntot = ((r1 + 2 - j0) / RING + 1) * RING;
+        qip = qw == 0 ? ny - 1 : qw - 1;
+        c0 = (strip * OUTW - 4) % nx;
+        if (c0 < 0) c0 += nx;
+        txbytes = (uint32_t)W * (uint32_t)(NC * sizeof(C) + (RES ? NC * sizeof(T) : 0) + (Vp ? sizeof(T) : 0) + (Pp ? sizeof(T) : 0) +
+                                           (DRIVE ? sizeof(C) : 0));
+    }
+    // issues fetch fi (psi row qi of every component, row-local inputs of row qip) into stage fi mod DEPTH; a strip that
+    // crosses the periodic x edge is copied in two pieces (the launch plan takes this path only for nx >= W)
+    const uint32_t lead = lane == 0;
+    const int len1 = min((int)W, nx - c0), len2 = W - len1;
+    auto issue_fetch = [&]() {
+        const uint32_t slot = (uint32_t)fi % DEPTH, bar = bar0 + slot * 8, dst = ring0 + slot * SM::STAGE;
+        mbar_expect_tx(bar, txbytes, lead);
+        const uint32_t eq = (uint32_t)qi * (uint32_t)nx, ep = (uint32_t)qip * (uint32_t)nx;
+#pragma unroll
+        for (int s = 0; s < NC; ++s) {
+            bulk_g2s(dst + SM::PSI + s * W * sizeof(C), pin[s] + eq + c0, len1 * sizeof(C), bar, lead);
+            if constexpr (RES) bulk_g2s(dst + SM::N + s * W * sizeof(T), nin[s] + ep + c0, len1 * sizeof(T), bar, lead);
+        }
+        if (Vp) bulk_g2s(dst + SM::V, Vp + ep + c0, len1 * sizeof(T), bar, lead);
+        if (Pp) bulk_g2s(dst + SM::P, Pp + ep + c0, len1 * sizeof(T), bar, lead);
+        if constexpr (DRIVE) bulk_g2s(dst + SM::E, Ep + ep + c0, len1 * sizeof(C), bar, lead);
+        if (len2 > 0) {
+#pragma unroll
+            for (int s = 0; s < NC; ++s) {
+                bulk_g2s(dst + SM::PSI + (s * W + len1) * sizeof(C), pin[s] + eq, len2 * sizeof(C), bar, lead);
+                if constexpr (RES) bulk_g2s(dst + SM::N + (s * W + len1) * sizeof(T), nin[s] + ep, len2 * sizeof(T), bar, lead);
+            }
+            if (Vp) bulk_g2s(dst + SM::V + len1 * sizeof(T), Vp + ep, len2 * sizeof(T), bar, lead);
+            if (Pp) bulk_g2s(dst + SM::P + len1 * sizeof(T), Pp + ep, len2 * sizeof(T), bar, lead);
+            if constexpr (DRIVE) bulk_g2s(dst + SM::E + len1 * sizeof(C), Ep + ep, len2 * sizeof(C), bar, lead);
+        }
+        ++fi;
+        qip = qi;
+        if (++qi == ny) qi = 0;
+    };
+    uint32_t ready = 0;                                 // has the stage of the next iteration landed? (tested one iteration early)
+    if constexpr (BULK) {
+        for (int d = 0; d < DEPTH - 1 && fi < ntot; ++d) issue_fetch();
+    }
+
     // ---- row loop: one pass = RING front rows j0 + RING*k + ph.  Each phase is straight-line code (no branch around the
     // fetch or the four stages), so that the scheduler sees the loads and their consumers in one block. -------------------------
 #define SL(d) ((ph + (d) + 2 * RING) % RING)     // ring slot of row j+d
@@ -301,7 +445,7 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
 #pragma unroll
         for (int ph = 0; ph < RING; ++ph) {
             const int j = jb + ph;          // front row of this iteration (rows past r1+2 in the last pass are computed and not stored)
-            if (PF > 0) {
+            if (PF > 0 && !BULK) {
                 if (!ZBC) {
                     uint32_t e = ew + epf;                   // row qw + pfr, wrapped
                     if (qw + pfr >= ny) e -= plane;
@@ -328,6 +472,22 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
             // Periodic: every (wrapped) row is readable, so the fetch is unconditional (rows past r1+3 are fetched and not
             // used).  Zero boundaries: a row or column outside the grid reads as 0.
             const bool okq = !ZBC || (inx && (j + 1 + LEAD <= r1 + 3) && (!zy || (qw >= 0 && qw < ny)));
+            if constexpr (BULK) {
+                // the stage of this iteration has landed (phase parity of its mbarrier); registers <- shared memory
+                const uint32_t slot = (uint32_t)fc % DEPTH;
+                if (!ready) mbar_wait(bar0 + slot * 8, ((uint32_t)fc / DEPTH) & 1u);     // (rare: the copies run DEPTH - 1 rows ahead)
+                const unsigned char* st = ringp + slot * SM::STAGE;
+#pragma unroll
+                for (int s = 0; s < NC; ++s) {
+                    ldsc<VEC>(reinterpret_cast<const C*>(st + SM::PSI) + s * W + lane * VEC, psr[s][SL(1 + LEAD)]);
+                    if constexpr (RES) ldsr<VEC>(reinterpret_cast<const T*>(st + SM::N) + s * W + lane * VEC, nr[s][SL(LEAD)]);
+                }
+                if (Vp) ldsr<VEC>(reinterpret_cast<const T*>(st + SM::V) + lane * VEC, Vr[SL(LEAD)]);
+                if (Pp) ldsr<VEC>(reinterpret_cast<const T*>(st + SM::P) + lane * VEC, Pr[SL(LEAD)]);
+                if constexpr (DRIVE) ldsc<VEC>(reinterpret_cast<const C*>(st + SM::E) + lane * VEC, Er[SL(LEAD)]);
+                ++fc;
+                ready = mbar_test(bar0 + ((uint32_t)fc % DEPTH) * 8, ((uint32_t)fc / DEPTH) & 1u);
+            } else {
 #pragma unroll
             for (int s = 0; s < NC; ++s) {
                 if (ZBC) {
@@ -354,6 +514,7 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
                     }
                     if (okprev) ldr<VEC>(nin[s] + ewp, nr[s][SL(LEAD)]);
                 }
+            }
             }
 
             {
@@ -432,6 +593,7 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
                 diffs(nb, df);
                 const int jr = j - 3;
                 const bool st_row = jr >= r0 && jr < r1;
+                uint4 wd_prev[VEC];                                 // the Philox words of a cell: (x, y) for psi_+, (z, w) for psi_-
 #pragma unroll
                 for (int s = 0; s < NC; ++s) {
                     C out[VEC];
@@ -444,17 +606,21 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
                         out[i] = fma2s(k.dt6, K, accr[s][SL(-3)][i]);
                         nout[i] = RES ? naccr[s][SL(-3)][i] + k.dt6 * Kn : T(0);
                     }
-                    if (st_row && st_lane) {
-                        if (NOISE) {
+                    if (NOISE) {
+                        // dW of Eq. (22), for every lane and row in straight-line code (no branch around it), so that the integer
+                        // work of Philox interleaves with the floating-point work of the stages; rows and lanes that are not
+                        // stored draw words nobody uses (the counter is the cell index, so nothing shifts)
 #pragma unroll
-                            for (int i = 0; i < VEC; ++i) {
-                                const uint32_t cell = (uint32_t)jr * (uint32_t)nx + (uint32_t)(xl + i);
-                                const uint4 wd = noise_words(a.seed, blockIdx.z, step, cell);
-                                const T nt = RES ? nr[s][SL(-3)][i] : T(0);      // reservoir at the start of the step
-                                const T var = k.sig2 * (T(2) * k.hgc + k.Rr * nt);
-                                out[i] = add2(out[i], s == 0 ? noise_increment(wd.x, wd.y, var) : noise_increment(wd.z, wd.w, var));
-                            }
+                        for (int i = 0; i < VEC; ++i) {
+                            const uint32_t cell = (uint32_t)jr * (uint32_t)nx + (uint32_t)(xl + i);
+                            const uint4 wd = s == 0 ? noise_words(a.seed, blockIdx.z, step, cell) : wd_prev[i];
+                            if (SPINOR && s == 0) wd_prev[i] = wd;
+                            const T nt = RES ? nr[s][SL(-3)][i] : T(0);      // reservoir at the start of the step
+                            const T var = k.sig2 * (T(2) * k.hgc + k.Rr * nt);
+                            out[i] = add2(out[i], s == 0 ? noise_increment_sfu(wd.x, wd.y, var) : noise_increment_sfu(wd.z, wd.w, var));
                         }
+                    }
+                    if (st_row && st_lane) {
                         stc<VEC>(pout[s] + est, out);
                         if constexpr (RES) str<VEC>(nout_p[s] + est, nout);
                     }
@@ -462,6 +628,12 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
             }
 
             // ---- next row -----------------------------------------------------------------------------------------------
+            if constexpr (BULK) {
+                // the stage read in the previous iteration is free (its registers were consumed by this iteration's stages):
+                // refill it with the row DEPTH - 1 iterations ahead
+                __syncwarp();
+                if (fi < ntot) issue_fetch();
+            }
             ewp = ew;
             okprev = okq;
             ++qw; ew += nx; est += nx;

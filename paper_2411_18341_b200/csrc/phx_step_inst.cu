@@ -40,19 +40,32 @@ typedef double real_t;
 #define PHX_HAS_VEC4 (PHX_INST_PREC == 32 && PHX_INST_MODEL == 0)
 #endif
 
-template <int VEC, bool NOISE, bool ZBC, bool ISO, bool DRIVE>
+template <int VEC, bool NOISE, bool ZBC, bool ISO, bool DRIVE, bool BULK>
 struct Inst {
     // (the noisy reservoir kernel, cfg5, is 9 % faster with the registers of 8 resident warps than with those of 12)
     static constexpr int MINW = VEC == 4 ? PHX_MINW_V4 : (VEC == 2 ? ((NOISE && PHX_INST_MODEL == 1 && PHX_INST_PREC == 32) ? 8 : PHX_MINW_V2) : PHX_MINW_V1);
     static constexpr bool I = ISO && PHX_HAS_ISO;
+    // dynamic shared memory: the per-warp rings of the bulk-copy fetch path
+    static constexpr size_t SMEM = BULK ? StepSmem<real_t, VEC, PHX_INST_MODEL, DRIVE>::CTA : 0;
+    static cudaError_t prepare() {
+        if (SMEM > 48 * 1024) {
+            static cudaError_t once = cudaFuncSetAttribute(step_kernel<real_t, VEC, PHX_INST_MODEL, NOISE, ZBC, I, DRIVE, MINW, BULK>,
+                                                           cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM);
+            return once;
+        }
+        return cudaSuccess;
+    }
     static cudaError_t launch(const StepArgs<real_t>& a, dim3 grid, cudaStream_t st) {
-        step_kernel<real_t, VEC, PHX_INST_MODEL, NOISE, ZBC, I, DRIVE, MINW><<<grid, 32 * PHX_STEP_WARPS, 0, st>>>(a);
+        cudaError_t e = prepare();
+        if (e != cudaSuccess) return e;
+        step_kernel<real_t, VEC, PHX_INST_MODEL, NOISE, ZBC, I, DRIVE, MINW, BULK><<<grid, 32 * PHX_STEP_WARPS, SMEM, st>>>(a);
         return cudaGetLastError();
     }
     static int occupancy() {   // resident CTAs per SM
         int nb = 0;
-        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, step_kernel<real_t, VEC, PHX_INST_MODEL, NOISE, ZBC, I, DRIVE, MINW>,
-                                                          32 * PHX_STEP_WARPS, 0) != cudaSuccess) {
+        if (prepare() != cudaSuccess ||
+            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, step_kernel<real_t, VEC, PHX_INST_MODEL, NOISE, ZBC, I, DRIVE, MINW, BULK>,
+                                                          32 * PHX_STEP_WARPS, SMEM) != cudaSuccess) {
             cudaGetLastError();
             return MINW / PHX_STEP_WARPS;
         }
@@ -61,59 +74,61 @@ struct Inst {
 };
 
 // The driven kernels are instantiated without noise (a driven noisy grid runs variant STAGE).
+// (the bulk-copy fetch path exists for periodic boundaries; a grid with a zero boundary takes the register loads)
 template <int VEC, bool NOISE, bool DRIVE, typename F>
-static auto dispatch2(bool zbc, bool iso, F f) {
-    if (zbc) return iso ? f(Inst<VEC, NOISE, true, true, DRIVE>()) : f(Inst<VEC, NOISE, true, false, DRIVE>());
-    return iso ? f(Inst<VEC, NOISE, false, true, DRIVE>()) : f(Inst<VEC, NOISE, false, false, DRIVE>());
+static auto dispatch2(bool zbc, bool iso, bool bulk, F f) {
+    if (zbc) return iso ? f(Inst<VEC, NOISE, true, true, DRIVE, false>()) : f(Inst<VEC, NOISE, true, false, DRIVE, false>());
+    if (bulk) return iso ? f(Inst<VEC, NOISE, false, true, DRIVE, true>()) : f(Inst<VEC, NOISE, false, false, DRIVE, true>());
+    return iso ? f(Inst<VEC, NOISE, false, true, DRIVE, false>()) : f(Inst<VEC, NOISE, false, false, DRIVE, false>());
 }
 
 template <int VEC, typename F>
-static auto dispatch(bool noise, bool zbc, bool iso, bool drive, F f) {
-    if (noise) return dispatch2<VEC, true, false>(zbc, iso, f);
-    if (drive) return dispatch2<VEC, false, true>(zbc, iso, f);
-    return dispatch2<VEC, false, false>(zbc, iso, f);
+static auto dispatch(bool noise, bool zbc, bool iso, bool drive, bool bulk, F f) {
+    if (noise) return dispatch2<VEC, true, false>(zbc, iso, bulk, f);
+    if (drive) return dispatch2<VEC, false, true>(zbc, iso, bulk, f);
+    return dispatch2<VEC, false, false>(zbc, iso, bulk, f);
 }
 
 template <int VEC>
-static int occ_vec(bool noise, bool zbc, bool iso, bool drive) {
-    return dispatch<VEC>(noise, zbc, iso, drive, [](auto inst) { return decltype(inst)::occupancy(); });
+static int occ_vec(bool noise, bool zbc, bool iso, bool drive, bool bulk) {
+    return dispatch<VEC>(noise, zbc, iso, drive, bulk, [](auto inst) { return decltype(inst)::occupancy(); });
 }
 
 template <int VEC>
-static cudaError_t launch_vec(const StepArgs<real_t>& a, bool noise, bool zbc, bool iso, dim3 grid, cudaStream_t st) {
-    return dispatch<VEC>(noise, zbc, iso, a.E != nullptr, [&](auto inst) { return decltype(inst)::launch(a, grid, st); });
+static cudaError_t launch_vec(const StepArgs<real_t>& a, bool noise, bool zbc, bool iso, bool bulk, dim3 grid, cudaStream_t st) {
+    return dispatch<VEC>(noise, zbc, iso, a.E != nullptr, bulk, [&](auto inst) { return decltype(inst)::launch(a, grid, st); });
 }
 
 #define PHX_CAT3(a, b, c) a##b##_##c
 #define PHX_NAME(p, m) PHX_CAT3(launch_step_, p, m)
 
-cudaError_t PHX_NAME(PHX_INST_PREC, PHX_INST_MODEL)(const StepArgs<real_t>& a, bool noise, bool zbc, bool iso, int vec,
+cudaError_t PHX_NAME(PHX_INST_PREC, PHX_INST_MODEL)(const StepArgs<real_t>& a, bool noise, bool zbc, bool iso, bool bulk, int vec,
                                                     dim3 grid, cudaStream_t st) {
 #if PHX_INST_PREC == 32
 #if PHX_HAS_VEC4
-    if (vec == 4) return launch_vec<4>(a, noise, zbc, iso, grid, st);
+    if (vec == 4) return launch_vec<4>(a, noise, zbc, iso, bulk, grid, st);
 #endif
-    if (vec == 2) return launch_vec<2>(a, noise, zbc, iso, grid, st);
+    if (vec == 2) return launch_vec<2>(a, noise, zbc, iso, bulk, grid, st);
 #elif PHX_HAS_VEC2_64
-    if (vec == 2) return launch_vec<2>(a, noise, zbc, iso, grid, st);
+    if (vec == 2) return launch_vec<2>(a, noise, zbc, iso, bulk, grid, st);
 #endif
-    if (vec == 1) return launch_vec<1>(a, noise, zbc, iso, grid, st);
+    if (vec == 1) return launch_vec<1>(a, noise, zbc, iso, bulk, grid, st);
     return cudaErrorInvalidValue;
 }
 
 #define PHX_OCC_NAME(p, m) PHX_CAT3(occupancy_step_, p, m)
 
 // Resident CTAs per SM of the instantiation (for the launch plan: one balanced wave).
-int PHX_OCC_NAME(PHX_INST_PREC, PHX_INST_MODEL)(bool noise, bool zbc, bool iso, bool drive, int vec) {
+int PHX_OCC_NAME(PHX_INST_PREC, PHX_INST_MODEL)(bool noise, bool zbc, bool iso, bool drive, bool bulk, int vec) {
 #if PHX_INST_PREC == 32
 #if PHX_HAS_VEC4
-    if (vec == 4) return occ_vec<4>(noise, zbc, iso, drive);
+    if (vec == 4) return occ_vec<4>(noise, zbc, iso, drive, bulk);
 #endif
-    if (vec == 2) return occ_vec<2>(noise, zbc, iso, drive);
+    if (vec == 2) return occ_vec<2>(noise, zbc, iso, drive, bulk);
 #elif PHX_HAS_VEC2_64
-    if (vec == 2) return occ_vec<2>(noise, zbc, iso, drive);
+    if (vec == 2) return occ_vec<2>(noise, zbc, iso, drive, bulk);
 #endif
-    return occ_vec<1>(noise, zbc, iso, drive);
+    return occ_vec<1>(noise, zbc, iso, drive, bulk);
 }
 
 }  // namespace phx

@@ -23,6 +23,7 @@ import pytest
 import oracle as orc
 from paper_2411_18341_b200 import workloads as wl
 from helpers import TOL, check_close, make_gpu, make_oracle
+from test_gpu_horizons import _report
 
 pytestmark = pytest.mark.gpu
 
@@ -156,7 +157,8 @@ def test_cfg5_realisations_0_255_511_for_500_steps():
             o.set_field(name, arr[r:r + 1])
         o.step_rk4(500)
         for name in w.fields:
-            check_close(got[name][r], getattr(o, name)[0], TOL["c32"], f"realisation {r} {name} after 500 steps")
+            err = check_close(got[name][r], getattr(o, name)[0], TOL["c32"], f"realisation {r} {name} after 500 steps")
+            _report(f"cfg5_512x256_r{r}_{name}_500", err)
 
 
 def test_cfg5_ensemble_mean_of_16_realisations_for_200_steps():
@@ -166,8 +168,9 @@ def test_cfg5_ensemble_mean_of_16_realisations_for_200_steps():
     g.step_rk4(200)
     o.step_rk4(200)
     for name in w.fields:
-        check_close(g.read_field(name), getattr(o, name), TOL["c32"], f"{w.name} {name} after 200 steps")
-    check_close(g.ensemble_mean_density("psi_p"), o.ensemble_mean_density("psi_p"), TOL["c32"], "ensemble mean, 200 steps")
+        _report(f"cfg5_16x256_{name}_200", check_close(g.read_field(name), getattr(o, name), TOL["c32"], f"{w.name} {name} after 200 steps"))
+    _report("cfg5_16x256_mean_200", check_close(g.ensemble_mean_density("psi_p"), o.ensemble_mean_density("psi_p"), TOL["c32"],
+                                                "ensemble mean, 200 steps"))
     g.destroy()
 
 

@@ -185,6 +185,11 @@ def test_cfg5_noisy_ensemble_reduced(prec):
 
 
 def test_noise_one_step_from_zero_matches_normal_map():
+    # psi = 0, n = 0: after one step psi is exactly sigma (xi1 + i xi2): the float Box-Muller map, cell by cell.
+    # The fused kernels evaluate it on the special-function unit (phx_philox.cuh, noise_increment_sfu): lg2.approx has a
+    # relative error of 2^-22, sin.approx / cos.approx an absolute error of 2^-20.9 = 5.1e-7 on [-pi, pi] (PTX ISA), and
+    # the angle 2 pi (u2 - 1/2) is rounded once (1.9e-7): an element is within 1e-6 of its own radius of the
+    # double-precision map, hence within 2e-6 of the largest one.  (The per-stage kernels keep logf / sincospif: 4e-7 there.)
     w = wl.cfg5(n=64, batch=3, prec="c32")
     w.fields["psi_p"][...] = 0
     g = make_gpu(w, variant=STEP)
@@ -192,7 +197,8 @@ def test_noise_one_step_from_zero_matches_normal_map():
     g.step_rk4(1)
     o.step_rk4(1)
     got = g.read_field("psi_p")
-    assert np.max(np.abs(got - o.psi_p)) <= 4e-7 * np.max(np.abs(o.psi_p))
+    assert np.max(np.abs(got - o.psi_p)) <= 2e-6 * np.max(np.abs(o.psi_p))
+    assert rel_l2(got, o.psi_p) <= 1e-6
     g.destroy()
 
 

@@ -4,8 +4,10 @@
     python bench.py [--gpus N] [--steps K] [--warmup W] [--workload NAME] [--variant V] [--impl reference]
 
 A "step" is one RK4 step (all four stages, plus noise where the workload has it) over the whole grid /
-ensemble.  `value` times K steps with the state resident in HBM (CUDA events on the launching stream,
-barrier + synchronize on both sides, max over ranks).  `e2e` times the same metric through the C ABI with
+ensemble.  `value` times blocks of exactly K steps with the state resident in HBM (CUDA events on the launching
+stream, barrier + synchronize on both sides, max over ranks): the block is repeated until the timed region is at
+least 0.5 s long (at least 5 blocks) and the MEDIAN block is reported, so that a short
+--steps does not turn the measurement into a millisecond sample.  `e2e` times the same metric through the C ABI with
 HOST buffers: every step uploads psi from pinned host memory, runs one RK4 step and downloads psi.
 The path does not shard (replicas only): with --gpus N each rank steps an independent
 replica of the workload and `value` is the sum.  Prints ONE JSON line on rank 0.
@@ -32,8 +34,11 @@ UNIT = "Gcell*step/s"
 COMPULSORY_BYTES = {"scalar": 20, "reservoir": 28, "spinor": 32, "spinor_reservoir": 52}
 
 
-def build_workload(name):
+def build_workload(name, quick=False):
+    """quick=True (the short other_workloads timings): the 16384^2 spinor fields are a 2048^2 recipe tile repeated 8 x 8."""
     from paper_2411_18341_b200 import workloads as wl
+    if quick and name == "cfg4_16384_c32":
+        return wl.cfg4(16384, "c32", tile=2048)
     table = {
         "cfg1": lambda: wl.cfg1(),
         "cfg2_1024_c32": lambda: wl.cfg2(1024, "c32"), "cfg2_1024_c64": lambda: wl.cfg2(1024, "c64"),
@@ -89,6 +94,24 @@ def algo_flops_per_cell_step(w):
     res = w.model.endswith("reservoir")
     per_stage = 33 + (9 if res else 0) + (36 if ncomp == 2 else 0)
     return ncomp * (4 * per_stage + 28 + (14 if res else 0))
+
+
+# SURVEY.md section 8(d)'s own flop count per cell-step (scalar 130, reservoir + 50, spinor 2 x 170), next to DESIGN.md's.
+SURVEY_FLOPS = {"scalar": 130, "reservoir": 180, "spinor": 340, "spinor_reservoir": 440}
+
+
+def read_traffic():
+    """profiles/traffic.csv: (workload, variant) -> (DRAM bytes per launch from the ncu capture, source)."""
+    out = {}
+    path = os.path.join(ROOT, "profiles", "traffic.csv")
+    if os.path.exists(path):
+        for line in open(path):
+            p = [x.strip() for x in line.split(",", 3)]
+            try:
+                out[(p[0], int(p[1]))] = (float(p[2]), p[3])
+            except (ValueError, IndexError):
+                continue
+    return out
 
 
 # Plain-ALU peak (no tensor cores: the stencil is not a contraction): 148 SMs x 128 FP32 (64 FP64) lanes x 2 flop x
@@ -169,9 +192,11 @@ def whole_job_value(world, cells, steps, ms):
     return world * cells * steps / (ms * 1e-3) / 1e9
 
 
-def oracle_from_workload(w, ny=None):
-    """The oracle as it stands on (a row-slab sample of) the workload."""
+def oracle_from_workload(w, ny=None, openmp=False):
+    """The oracle as it stands on (a row-slab sample of) the workload.  openmp=True: the same source built with its
+    OpenMP pragmas honoured (all host cores; the parity oracle is the single-threaded build)."""
     import oracle as orc
+    orc.select_build(openmp)
     ny = w.ny if ny is None else ny
     o = orc.Oracle(w.nx, ny, w.dx, w.dy, orc.make_params(**w.params), model=w.model, batch=1, prec32=(w.prec == "c32"),
                    noise=w.noise, seed=w.seed, V=None if w.V is None else w.V[:ny].astype(np.float64),
@@ -220,6 +245,8 @@ def main():
     ap.add_argument("--variant", type=int, default=0)
     ap.add_argument("--tune", default="", help="comma separated key=value passed to phx_set_tuning")
     ap.add_argument("--e2e-steps", type=int, default=20)
+    ap.add_argument("--min-seconds", type=float, default=0.5, help="floor of the timed region (blocks of --steps steps)")
+    ap.add_argument("--no-other-workloads", action="store_true", help="skip the short timings of the other BASELINE configs")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-stage-leg", action="store_true", help="skip the extra timing of variant STAGE")
     args = ap.parse_args()
@@ -256,17 +283,36 @@ def main():
             torch.cuda.synchronize()
 
     # ---- device-resident throughput ---------------------------------------------------------------------
-    def timed(steps):
+    def timed(gr, steps):
         """CUDA events on the launching stream around `steps` RK4 steps, barrier + synchronize on both sides."""
-        launches0 = g.get_launch_count()
+        launches0 = gr.get_launch_count()
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         barrier()
         e0.record(stream)
-        g.step_rk4(steps)
+        gr.step_rk4(steps)
         e1.record(stream)
         barrier()
         t_ms = max_over_ranks(e0.elapsed_time(e1), world)
-        return t_ms, g.get_launch_count() - launches0
+        return t_ms, gr.get_launch_count() - launches0
+
+    def timed_blocks(gr, steps, min_seconds, min_blocks=5, max_blocks=4000):
+        """Blocks of exactly `steps` steps back to back on the stream, each bracketed by CUDA events, the whole region by
+        barrier + synchronize; returns (median block ms (max over ranks), launches in the region, blocks, region ms)."""
+        t1, _ = timed(gr, steps)                               # sizes the region (and is one more warm-up)
+        nb = int(min(max_blocks, max(min_blocks, np.ceil(min_seconds * 1e3 / max(t1, 1e-3)))))
+        if world > 1:                                          # every rank runs the same number of blocks
+            nb = int(max_over_ranks(nb, world))
+        launches0 = gr.get_launch_count()
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(nb + 1)]
+        barrier()
+        ev[0].record(stream)
+        for b in range(nb):
+            gr.step_rk4(steps)
+            ev[b + 1].record(stream)
+        barrier()
+        blocks_ms = [ev[b].elapsed_time(ev[b + 1]) for b in range(nb)]
+        med = max_over_ranks(statistics.median(blocks_ms), world)
+        return med, gr.get_launch_count() - launches0, nb, max_over_ranks(ev[0].elapsed_time(ev[nb]), world)
 
     g.step_rk4(args.warmup)
     barrier()
@@ -275,11 +321,12 @@ def main():
         sampler.start()
         time.sleep(0.25)
     t_wall0 = time.time()
-    ms, launches = timed(args.steps)
+    ms, launches, n_blocks, region_ms = timed_blocks(g, args.steps, args.min_seconds)
     t_wall1 = time.time()
     clocks = sampler.stop(t_wall0, t_wall1) if rank == 0 else None
     cells = w.cells
     value = whole_job_value(world, cells, args.steps, ms)
+    launches_per_block = launches / n_blocks
 
     # the per-stage variant (the HBM-bound kernels of the north_star's >= 70 % target), timed the same way on a
     # shorter run, when the headline ran the fused step
@@ -288,7 +335,8 @@ def main():
         g.select_variant(phx.PHX_VARIANT_STAGE)
         g.step_rk4(args.warmup)
         st_steps = max(8, args.steps // 4)
-        st_ms, st_launches = timed(st_steps)
+        st_ms, st_launches, st_blocks, _ = timed_blocks(g, st_steps, args.min_seconds / 2)
+        st_launches //= st_blocks
         st_bpc = algo_bytes_per_cell_step(w, phx.PHX_VARIANT_STAGE)
         st_val = whole_job_value(world, cells, st_steps, st_ms)
         st_gbs = st_bpc * cells * st_steps / (st_ms * 1e-3) / 1e9
@@ -298,6 +346,7 @@ def main():
                       "roofline": {"bound": "hbm", "achieved": st_gbs, "unit": "GB/s"}}
         g.select_variant(variant)
     finite = bool(np.all(np.isfinite(g.read_field("psi_p")[0, :4])))
+    ws_bytes = g.workspace.numel()
 
     # ---- end to end through the C ABI with host buffers ----------------------------------------------------
     # Every step uploads its state from pinned host memory, runs one RK4 step and downloads the result.  Two handles on two
@@ -346,57 +395,108 @@ def main():
         return
 
     # ---- roofline of the dominant kernel ------------------------------------------------------------------------
+    # Primary: the HBM roof (the lower roof of the model: 130-160 flop per 20 B is below the machine balance of 11 flop/B)
+    # with the ALGORITHMIC bytes of the kernel that ran: achieved = bytes per launch / average launch duration.
     peak, peak_src = measured_peaks()
     bpc = algo_bytes_per_cell_step(w, variant, args.steps)
-    kernels_per_step = launches / args.steps
+    kernels_per_step = launches_per_block / args.steps
     bytes_per_launch = bpc * cells / kernels_per_step
-    launch_ms = ms / launches
+    launch_ms = ms / launches_per_block
     achieved = bytes_per_launch / (launch_ms * 1e-3) / 1e9
     comp = COMPULSORY_BYTES[w.model] * (2 if w.prec == "c64" else 1)
     kernel = {1: "phx::stage_kernel (4 launches per step)", 3: "phx::step_kernel (1 launch per step)",
               4: "phx::resident_kernel (1 launch for all steps)"}.get(variant, str(variant))
-    hbm = {"achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "peak_source": peak_src,
-           "algorithmic_bytes_per_cell_step": bpc, "bytes_per_launch": bytes_per_launch,
-           "compulsory_bytes_per_cell_step": comp, "compulsory_frac": value / world * 1e9 * comp / 1e9 / peak}
+    roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": None,
+                "peak_source": peak_src, "kernel": kernel, "avg_launch_ms": launch_ms,
+                "algorithmic_bytes_per_cell_step": bpc, "bytes_per_launch": bytes_per_launch,
+                "compulsory_bytes_per_cell_step": comp, "compulsory_frac": value / world * 1e9 * comp / 1e9 / peak}
     if variant in (phx.PHX_VARIANT_STEP, phx.PHX_VARIANT_RESIDENT):
-        # the fused step moves the compulsory bytes only; it is bound by plain FP32/FP64 instruction issue
+        # what actually limits the fused kernels is FP32/FP64 instruction issue: the same run against the
+        # plain-ALU peak, nested; flops as SURVEY.md 8(d) counts them (130 per scalar cell-step) and as DESIGN.md counts them
         fpc = algo_flops_per_cell_step(w)
         alu_peak = ALU_PEAK_TFLOPS[w.prec]
         tf = fpc * cells / kernels_per_step / (launch_ms * 1e-3) / 1e12
-        roofline = {"bound": "alu", "achieved": tf, "peak": alu_peak, "unit": "TFLOP/s", "frac": tf / alu_peak,
-                    "traffic": None, "peak_source": "derived: 148 SM x 128 (fp64: 64) lanes x 2 x 1.965 GHz, no tensor cores",
-                    "kernel": kernel, "algorithmic_flops_per_cell_step": fpc, "flops_per_launch": fpc * cells / kernels_per_step,
-                    "avg_launch_ms": launch_ms, "hbm": hbm}
-    else:
-        roofline = dict(hbm, bound="hbm", traffic=None, kernel=kernel, avg_launch_ms=launch_ms)
+        roofline["alu"] = {"achieved": tf, "peak": alu_peak, "unit": "TFLOP/s", "frac": tf / alu_peak,
+                           "peak_source": "derived: 148 SM x 128 (fp64: 64) lanes x 2 x 1.965 GHz, no tensor cores",
+                           "algorithmic_flops_per_cell_step": fpc,
+                           "frac_with_survey_flop_count": tf / alu_peak * SURVEY_FLOPS.get(w.model, fpc) / fpc}
+    # DRAM bytes per launch of this kernel from the committed `ncu --set full` captures (profiles/traffic.csv)
+    traffic = read_traffic()
+    if (args.workload, variant) in traffic:
+        roofline["traffic"], roofline["traffic_source"] = traffic[(args.workload, variant)]
+        roofline["frac_ncu_bytes"] = roofline["traffic"] / (launch_ms * 1e-3) / 1e9 / peak
+    hbm_target = None
     if stage_info is not None:
-        stage_info["roofline"].update(peak=peak, frac=stage_info["roofline"]["achieved"] / peak, peak_source=peak_src)
-    # DRAM bytes per launch of this kernel from the committed `ncu --set full` capture (profiles/traffic.csv)
-    traffic_file = os.path.join(ROOT, "profiles", "traffic.csv")
-    if os.path.exists(traffic_file):
-        try:
-            for line in open(traffic_file):
-                p = [x.strip() for x in line.split(",")]
-                if len(p) >= 4 and p[0] == args.workload and p[1] == str(variant):
-                    roofline["traffic"] = float(p[2])
-                    roofline["traffic_source"] = p[3]
-        except Exception:
-            pass
+        r = stage_info["roofline"]
+        r.update(peak=peak, frac=r["achieved"] / peak, peak_source=peak_src)
+        if (args.workload, 1) in traffic:
+            tb, src = traffic[(args.workload, 1)]
+            r["traffic"], r["traffic_source"] = tb, src
+            r["frac_ncu_bytes"] = tb / (stage_info["ms_per_step"] / 4 * 1e-3) / 1e9 / peak
+        # the north_star target (>= 70 % of the HBM roofline, bytes per cell-step from the ncu counters) is written for the
+        # per-stage kernels; the fused step moves 6.4x fewer bytes and is judged by compulsory_frac / the ALU fraction
+        f_ncu = r.get("frac_ncu_bytes")
+        hbm_target = {"variant": 1, "frac_algorithmic_bytes": r["frac"], "frac_ncu_bytes": f_ncu,
+                      "met": bool((f_ncu if f_ncu is not None else r["frac"]) >= 0.70)}
 
-    # ---- the oracle timed on this box's host cores (bounded sample) -----------------------------------------------
+    # ---- short timings of the other BASELINE configs (STEP / AUTO and STAGE), so that every size the north_star names is
+    # driver-visible: cfg4 16384^2, cfg3, cfg5, cfg2 fp64 (about 0.2 s of GPU time each) -------------------------------------
+    others = None
+    if not args.no_other_workloads and world == 1 and args.workload == "cfg2_4096_c32":
+        others = {}
+        g.destroy()
+        del g
+        torch.cuda.empty_cache()
+        for name in ("cfg2_4096_c64", "cfg3_4096_c32", "cfg5_512x256_c32", "cfg4_16384_c32", "cfg2_1024_c32"):
+            ow = build_workload(name, quick=True)
+            og = phx.grid_from_workload(ow, stream=stream, device=f"cuda:{local}")
+            rec = {}
+            for vname, v in (("auto", phx.PHX_VARIANT_AUTO), ("stage", phx.PHX_VARIANT_STAGE)):
+                og.select_variant(v)
+                vv = og.get_variant()
+                og.step_rk4(5)
+                o_steps = 16 if name.startswith("cfg4") else 64
+                o_ms, o_l, o_nb, _ = timed_blocks(og, o_steps, 0.2)
+                val = ow.cells * o_steps / (o_ms * 1e-3) / 1e9
+                ob = algo_bytes_per_cell_step(ow, vv, o_steps)
+                oc = COMPULSORY_BYTES[ow.model] * (2 if ow.prec == "c64" else 1)
+                rec[vname] = {"variant": vv, "value": val, "unit": UNIT, "ms_per_step": o_ms / o_steps, "steps": o_steps,
+                              "blocks": o_nb, "algorithmic_bytes_per_cell_step": ob, "hbm_frac": val * ob / peak,
+                              "compulsory_frac": val * oc / peak}
+                if (name, vv) in traffic:
+                    kps = o_l / o_nb / o_steps
+                    rec[vname]["hbm_frac_ncu_bytes"] = traffic[(name, vv)][0] * kps / (o_ms / o_steps * 1e-3) / 1e9 / peak
+            rec["finite"] = bool(np.all(np.isfinite(og.read_field("psi_p")[0, :2])))
+            others[name] = rec
+            og.destroy()
+            del og, ow
+            torch.cuda.empty_cache()
+
+    # ---- the oracle timed on this box's host cores (bounded samples): as it stands on one core, and the same source with
+    # its OpenMP pragmas honoured on all cores ----------------------------------------------------------
     cpu = None
     if not args.no_cpu_baseline and world == 1:
         ny = max(3, min(w.ny, (1 << 22) // w.nx))              # ~4M cells per step, ~0.4 s per step
-        o = oracle_from_workload(w, ny)
-        o.step_rk4(1)
-        t0 = time.perf_counter()
-        nst = 0
-        while time.perf_counter() - t0 < 12.0:
+
+        def time_oracle(openmp, budget):
+            o = oracle_from_workload(w, ny, openmp=openmp)
             o.step_rk4(1)
-            nst += 1
-        dtc = time.perf_counter() - t0
-        cpu = {"value": w.nx * ny * nst / dtc / 1e9, "unit": UNIT, "cores": 1, "kind": "oracle",
-               "sample": f"{w.nx}x{ny} row slab of realisation 0, {nst} RK4 steps, fp64, single thread"}
+            t0 = time.perf_counter()
+            nst = 0
+            while time.perf_counter() - t0 < budget:
+                o.step_rk4(1)
+                nst += 1
+            return w.nx * ny * nst / (time.perf_counter() - t0) / 1e9, nst
+        v1, n1 = time_oracle(False, 10.0)
+        ncores = len(os.sched_getaffinity(0))
+        os.environ.setdefault("OMP_NUM_THREADS", str(ncores))
+        vn, nn_ = time_oracle(True, 8.0)
+        import oracle as orc
+        orc.select_build(False)
+        cpu = {"value": v1, "unit": UNIT, "cores": 1, "kind": "oracle",
+               "sample": f"{w.nx}x{ny} row slab of realisation 0, {n1} RK4 steps, fp64, single thread",
+               "all_cores": {"value": vn, "unit": UNIT, "cores": ncores, "kind": "oracle, OpenMP over the rows of each full-grid loop",
+                             "sample": f"{w.nx}x{ny} row slab, {nn_} RK4 steps"}}
 
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
@@ -404,14 +504,16 @@ def main():
         "dtype": "f32" if w.prec == "c32" else "f64", "data": "synthetic",
         "config": {"workload": args.workload, "model": None, "grid": [w.nx, w.ny], "batch": w.batch, "precision": w.prec,
                    "variant": variant, "parallelism": "replicas only" if world > 1 else "single GPU",
-                   "l2": f"working set {g.workspace.numel() / 2**20:.0f} MiB > 126 MB L2, no flush needed"
-                   if g.workspace.numel() > 200e6 else "working set fits L2 (L2-resident regime, reported as such)",
+                   "l2": f"working set {ws_bytes / 2**20:.0f} MiB > 126 MB L2, no flush needed"
+                   if ws_bytes > 200e6 else "working set fits L2 (L2-resident regime, reported as such)",
                    "finite": finite},
-        "clocks": clocks, "gpu_launches": int(launches),
+        "timed_blocks": n_blocks, "timed_region_ms": region_ms, "block": "median of the blocks of `steps` steps",
+        "clocks": clocks, "gpu_launches": int(launches), "gpu_launches_per_block": launches_per_block,
         "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                 "rk4_steps_per_call": 1, "steps": args.e2e_steps, "finite": e2e_finite,
                 "pipeline": "two handles on two streams: the upload of one step overlaps the download of the previous one"},
-        "roofline": roofline, "cpu_baseline": cpu, "stage_variant": stage_info,
+        "roofline": roofline, "cpu_baseline": cpu, "stage_variant": stage_info, "hbm_target": hbm_target,
+        "other_workloads": others,
     }
     del out["config"]["model"]
     print(json.dumps(out))

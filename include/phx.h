@@ -61,11 +61,11 @@ typedef enum { PHX_BC_PERIODIC = 0, PHX_BC_ZERO = 1 } phx_boundary;   /* PAPER.m
 
 /* Kernel variants (all compute the same RK4 step; they differ in how often data crosses HBM). */
 typedef enum {
-    PHX_VARIANT_AUTO = 0,      /* the fastest variant that can run the grid: RESIDENT for ensembles (batch >= 32) of grids that fit it, else STEP,
-                                  or STAGE for a driven grid with noise */
+    PHX_VARIANT_AUTO = 0,      /* the fastest variant that can run the grid: RESIDENT for ensembles (batch >= 32) of grids that fit it, else STEP
+                                  (STAGE for planes of 2^31 cells or more) */
     PHX_VARIANT_STAGE = 1,     /* one fused kernel per RK stage (4 launches per step); every model and term */
     PHX_VARIANT_STEP = 3,      /* one kernel per RK4 step: the four stages pipelined along y in register windows of
-                                  a haloed warp-wide column strip (N_halo = 4); not for drive + noise together */
+                                  a haloed warp-wide column strip (N_halo = 4); every model and term */
     PHX_VARIANT_RESIDENT = 4   /* grids of at most 64 x 64 cells (scalar and reservoir models, no drive): one CTA per
                                   realisation keeps the grid on chip for all steps of a phx_step_rk4 call (one launch) */
 } phx_variant;

@@ -32,10 +32,21 @@ class _Problem(C.Structure):
 _lib = None
 
 
+_omp = False
+
+
+def select_build(openmp: bool):
+    """openmp=True: use liboracle_omp.so (the same source with its OpenMP pragmas honoured) -- bench.py's all-cores
+    cpu_baseline leg only; the parity oracle is the single-threaded build (the default)."""
+    global _lib, _omp
+    if bool(openmp) != _omp:
+        _lib, _omp = None, bool(openmp)
+
+
 def lib():
     global _lib
     if _lib is None:
-        _lib = C.CDLL(_build.build())
+        _lib = C.CDLL(_build.build_omp() if _omp else _build.build())
         _lib.orc_step_rk4.restype = C.c_int32
         _lib.orc_step_rk4.argtypes = [C.c_void_p] * 5 + [C.c_uint64, C.c_int64]
         _lib.orc_derivative.restype = None

@@ -87,6 +87,7 @@ struct phx_grid {
     int rows, vec, graph_steps, gsteps;
     int parity;             // variant STEP ping-pongs the state: 0 = state in psi/n, 1 = state in ya/na
     int step_ly, step_vec;  // variant STEP geometry (0 = automatic)
+    int step_warps;         // variant STEP warps per CTA (0 = automatic)
     int step_bulk;          // variant STEP fetch path: -1 automatic, 0 register loads, 1 bulk copies into a shared-memory ring
     int async_host;         // 1: host copies of set_field / read_field do not synchronise (pinned buffers, caller syncs)
     cudaGraphExec_t g1[2], gN;  // one step from parity 0 / 1; graph_steps steps from parity 0
@@ -276,6 +277,18 @@ int step_occupancy(const phx_grid* g, int vec) {
     }
 }
 
+int step_strips(const phx_grid* g, int vec) { return (g->d.nx + 32 * vec - 9) / (32 * vec - 8); }
+
+// Warps per CTA: the warps of a CTA own adjacent strips and are otherwise independent.  Two per CTA measured 4 % faster
+// than one on the 16384^2 spinor and equal on the 4096^2 reservoir grid; but a row with an odd number of strips leaves the
+// last CTA's second warp idle: 1 of 6 warp slots on the 256-wide grids of cfg5 (5 strips: 91 against 75 Gcell*step/s with
+// one warp per CTA), 1 of 36 at 4096^2 scalar fp32 (+1.4 %).  One warp per CTA when more than 2 % of the slots would idle.
+int step_warps(const phx_grid* g, int vec) {
+    if (g->step_warps) return g->step_warps;
+    const int strips = step_strips(g, vec);
+    return (strips % PHX_STEP_WARPS != 0 && strips < 50) ? 1 : PHX_STEP_WARPS;
+}
+
 // Bytes one step of variant STEP touches per cell (state in and out, V, P, E).
 size_t step_bytes_per_cell(const phx_grid* g) {
     const size_t rb = real_bytes(g);
@@ -298,9 +311,9 @@ size_t step_bytes_per_cell(const phx_grid* g) {
 //    Gcell*step/s).
 int step_rows_per_chunk(const phx_grid* g, int vec) {
     if (g->step_ly) return g->step_ly < g->d.ny ? g->step_ly : g->d.ny;
-    const int strips = (g->d.nx + 32 * vec - 9) / (32 * vec - 8);
-    const long ctas_row = (long)((strips + PHX_STEP_WARPS - 1) / PHX_STEP_WARPS) * g->d.batch;
-    const long slots = (long)g->n_sm * step_occupancy(g, vec);
+    const int strips = step_strips(g, vec), wpc = step_warps(g, vec);
+    const long ctas_row = (long)((strips + wpc - 1) / wpc) * g->d.batch;
+    const long slots = (long)g->n_sm * step_occupancy(g, vec) * (PHX_STEP_WARPS / wpc);   // resident CTAs of wpc warps
     const bool in_l2 = plane_cells(g) * g->d.batch * step_bytes_per_cell(g) < g->l2_bytes / 2;
     double best_cost = -1;
     int best_ly = g->d.ny;
@@ -314,7 +327,7 @@ int step_rows_per_chunk(const phx_grid* g, int vec) {
         double cost = (double)(waves * iters);
         if (in_l2) {
             const long per_sm = ((ctas + waves - 1) / waves + g->n_sm - 1) / g->n_sm;     // CTAs on the fullest SM
-            const long per_sched = (per_sm * PHX_STEP_WARPS + 3) / 4;
+            const long per_sched = (per_sm * wpc + 3) / 4;
             cost *= per_sched > 1.75 ? (double)per_sched : 1.75;
         }
         if (best_cost < 0 || cost < best_cost) { best_cost = cost; best_ly = ly; }
@@ -351,9 +364,10 @@ cudaError_t enqueue_step_fused(phx_grid* g, cudaStream_t st, int parity) {
     a.step_out = slots + (1 - parity);
     a.seed = g->prm.seed;
     const int vec = step_vec(g);
-    a.strips = (g->d.nx + 32 * vec - 9) / (32 * vec - 8);
+    a.strips = step_strips(g, vec);
+    a.wpc = step_warps(g, vec);
     a.ly = step_rows_per_chunk(g, vec);
-    const dim3 grid((a.strips + PHX_STEP_WARPS - 1) / PHX_STEP_WARPS, (g->d.ny + a.ly - 1) / a.ly, g->d.batch);
+    const dim3 grid((a.strips + a.wpc - 1) / a.wpc, (g->d.ny + a.ly - 1) / a.ly, g->d.batch);
     if (grid.y > 65535u) return cudaErrorInvalidConfiguration;
     const bool noise = g->d.noise != 0, zbc = g->d.bc_x || g->d.bc_y, iso = step_iso(g), bulk = step_bulk(g);
     if constexpr (sizeof(T) == 4) {
@@ -419,10 +433,8 @@ cudaError_t capture(phx_grid* g, int steps, int parity, cudaGraphExec_t* out) {
     return e;
 }
 
-// The fused step addresses a plane by 32-bit cell offsets; its driven kernels are built without noise.
-bool step_variant_ok(const phx_grid* g) {
-    return !(g->hasE && g->d.noise) && (size_t)g->d.nx * (size_t)g->d.ny < ((size_t)1 << 31);
-}
+// The fused step addresses a plane by 32-bit cell offsets.
+bool step_variant_ok(const phx_grid* g) { return (size_t)g->d.nx * (size_t)g->d.ny < ((size_t)1 << 31); }
 
 // Variant RESIDENT: scalar and reservoir models without drive whose grid fits one CTA (phx_resident.cu).
 bool resident_variant_ok(const phx_grid* g) {
@@ -534,6 +546,7 @@ phx_status phx_create_grid(phx_grid** out, const phx_grid_desc* desc) {
     g->parity = 0;
     g->step_ly = g->step_vec = 0;
     g->step_bulk = -1;
+    g->step_warps = 0;
     g->async_host = 0;
     g->n_sm = prop.multiProcessorCount;
     g->l2_bytes = (size_t)prop.l2CacheSize;
@@ -775,6 +788,9 @@ phx_status phx_set_tuning(phx_grid* g, const char* key, int32_t value) {
         if (value == 4 && (g->d.model != PHX_SCALAR || g->d.prec != PHX_C32)) return fail(g, PHX_ERR_UNSUPPORTED, "step_vec=4 exists for the scalar fp32 model only");
         if (value == 2 && g->d.prec == PHX_C64 && g->d.model != PHX_SCALAR) return fail(g, PHX_ERR_UNSUPPORTED, "step_vec=2 in fp64 exists for the scalar model only");
         g->step_vec = value;
+    } else if (!std::strcmp(key, "step_warps")) {     // variant STEP: warps per CTA (0 = automatic)
+        if (value < 0 || value > PHX_STEP_WARPS) return PHX_ERR_INVALID_ARG;
+        g->step_warps = value;
     } else if (!std::strcmp(key, "step_bulk")) {      // variant STEP fetch path: -1 automatic, 0 register loads, 1 bulk copies
         if (value < -1 || value > 1) return PHX_ERR_INVALID_ARG;
         g->step_bulk = value;

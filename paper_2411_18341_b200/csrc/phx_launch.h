@@ -3,7 +3,8 @@
 
 #include "phx_common.cuh"
 
-// Warps per CTA of variant STEP (the warps of a CTA are independent: adjacent strips, no shared memory, no barrier).
+// Most warps per CTA of variant STEP (the warps of a CTA are independent: adjacent strips, no barrier between them; the
+// launch plan takes 1 or PHX_STEP_WARPS per CTA, whichever leaves fewer warp slots idle: StepArgs::wpc).
 #ifndef PHX_STEP_WARPS
 #define PHX_STEP_WARPS 2
 #endif

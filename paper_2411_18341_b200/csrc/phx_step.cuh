@@ -46,6 +46,7 @@ struct StepArgs {
     uint32_t seed;
     int ly;                     // rows per chunk
     int strips;                 // strips per row of the grid
+    int wpc;                    // warps per CTA of this launch (1 .. PHX_STEP_WARPS; the warps of a CTA are independent)
 };
 
 namespace stepk {
@@ -235,7 +236,7 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
     const int nx = g.nx, ny = g.ny;
 
     const int lane = threadIdx.x & 31;
-    const int strip = blockIdx.x * PHX_STEP_WARPS + (threadIdx.x >> 5);
+    const int strip = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
     const uint64_t step = *a.step_in;
     if (blockIdx.x == 0 && blockIdx.y == 0 && blockIdx.z == 0 && threadIdx.x == 0) *a.step_out = step + 1;
     if (strip >= a.strips) return;   // warp-uniform

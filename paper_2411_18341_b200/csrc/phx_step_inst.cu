@@ -58,10 +58,10 @@ struct Inst {
     static cudaError_t launch(const StepArgs<real_t>& a, dim3 grid, cudaStream_t st) {
         cudaError_t e = prepare();
         if (e != cudaSuccess) return e;
-        step_kernel<real_t, VEC, PHX_INST_MODEL, NOISE, ZBC, I, DRIVE, MINW, BULK><<<grid, 32 * PHX_STEP_WARPS, SMEM, st>>>(a);
+        step_kernel<real_t, VEC, PHX_INST_MODEL, NOISE, ZBC, I, DRIVE, MINW, BULK><<<grid, 32 * a.wpc, SMEM, st>>>(a);
         return cudaGetLastError();
     }
-    static int occupancy() {   // resident CTAs per SM
+    static int occupancy() {   // resident CTAs of PHX_STEP_WARPS warps per SM (the register file bounds the WARPS)
         int nb = 0;
         if (prepare() != cudaSuccess ||
             cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, step_kernel<real_t, VEC, PHX_INST_MODEL, NOISE, ZBC, I, DRIVE, MINW, BULK>,
@@ -73,7 +73,6 @@ struct Inst {
     }
 };
 
-// The driven kernels are instantiated without noise (a driven noisy grid runs variant STAGE).
 // (the bulk-copy fetch path exists for periodic boundaries; a grid with a zero boundary takes the register loads)
 template <int VEC, bool NOISE, bool DRIVE, typename F>
 static auto dispatch2(bool zbc, bool iso, bool bulk, F f) {
@@ -84,6 +83,7 @@ static auto dispatch2(bool zbc, bool iso, bool bulk, F f) {
 
 template <int VEC, typename F>
 static auto dispatch(bool noise, bool zbc, bool iso, bool drive, bool bulk, F f) {
+    if (noise && drive) return dispatch2<VEC, true, true>(zbc, iso, bulk, f);   // Eq. (16) carries E and dW together
     if (noise) return dispatch2<VEC, true, false>(zbc, iso, bulk, f);
     if (drive) return dispatch2<VEC, false, true>(zbc, iso, bulk, f);
     return dispatch2<VEC, false, false>(zbc, iso, bulk, f);

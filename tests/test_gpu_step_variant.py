@@ -142,8 +142,7 @@ def test_coherent_drive_cells_per_lane_and_boundaries(tuning, bc):
     run_pair(w, 60, E=_drive_field(w), extra_params=dict(omega=-2.1), tuning=tuning, bc=bc)
 
 
-def test_drive_set_mid_run_and_driven_noise_falls_back_to_stage():
-    from paper_2411_18341_b200 import binding as phx
+def test_drive_set_mid_run_and_drive_with_noise():
     w = wl.cfg2(n=64, ny=32, prec="c32")
     E = _drive_field(w)
     xp = dict(omega=1.3)
@@ -160,14 +159,16 @@ def test_drive_set_mid_run_and_driven_noise_falls_back_to_stage():
     o2.step_rk4(2)
     assert rel_l2(g.read_field("psi_p"), o2.psi_p) <= TOL["c32"]
     g.destroy()
-    # a driven grid with noise: the driven fused kernels are built without noise, AUTO takes the per-stage kernels
-    wn = wl.cfg5(n=64, batch=2)
-    gn = make_gpu(wn, E=_drive_field(wn))
-    assert gn.get_variant() == STAGE
-    with pytest.raises(phx.PhxError) as e:
-        gn.select_variant(STEP)
-    assert e.value.status == phx.PHX_ERR_UNSUPPORTED
-    gn.destroy()
+    # Eq. (16) carries E and dW together: a driven grid with noise runs the fused step as well
+    for wn in (wl.cfg5(n=64, batch=2), dataclasses.replace(wl.cfg4(n=96, prec="c32", sigma_cells=10.0), noise=True, seed=11)):
+        En = _drive_field(wn)
+        gn = make_gpu(wn, E=En, extra_params=xp)
+        assert gn.get_variant() == STEP
+        on = make_oracle(wn, E=En, extra_params=xp)
+        gn.step_rk4(25)
+        on.step_rk4(25)
+        compare(gn, on, wn)
+        gn.destroy()
 
 
 # ---- stochastic path -------------------------------------------------------------------------------------

@@ -58,6 +58,9 @@ typedef enum { PHX_SCALAR = 0, PHX_RESERVOIR = 1, PHX_SPINOR = 2, PHX_SPINOR_RES
 typedef enum { PHX_HOST = 0, PHX_DEVICE = 1 } phx_mem;
 typedef enum { PHX_PSI = 0, PHX_PSI_MINUS = 1, PHX_N = 2, PHX_N_MINUS = 3 } phx_field;
 typedef enum { PHX_BC_PERIODIC = 0, PHX_BC_ZERO = 1 } phx_boundary;
+/* PHX_INT_DP54 reserves the seven K buffers of the adaptive Dormand-Prince 5(4) integrator in the workspace
+ * (phx_step_adaptive).  phx_step_rk4 works on either kind of handle. */
+typedef enum { PHX_INT_RK4 = 0, PHX_INT_DP54 = 1 } phx_integrator;
 
 /* Kernel variants (all compute the same RK4 step; they differ in how often data crosses HBM). */
 typedef enum {
@@ -78,6 +81,7 @@ typedef struct {
     int32_t model;             /* phx_model */
     int32_t noise;             /* 0/1: add the Wiener increment of Eq. (22) after every step */
     int32_t bc_x, bc_y;        /* phx_boundary per axis */
+    int32_t integrator;        /* phx_integrator */
     void* workspace;           /* DEVICE memory owned by the caller, 256-byte aligned */
     size_t workspace_bytes;    /* >= phx_workspace_bytes(desc) */
     void* stream;              /* cudaStream_t owned by the caller; NULL = legacy default stream */
@@ -142,6 +146,42 @@ phx_status phx_read_field(phx_grid* g, phx_field f, void* dst, phx_mem where);
  * replayed from CUDA graphs; asynchronous on the stream, no host synchronisation.
  * INVALID_ARG: n_steps < 0; BAD_STATE: phx_set_params not called yet; CUDA: a launch failed (sticky). */
 phx_status phx_step_rk4(phx_grid* g, int64_t n_steps);
+
+/* ---- adaptive time stepping: Dormand-Prince 5(4) ----------------------------------------------------------------------
+ * "Higher-order methods like the RK-Fehlberg or Dormand-Prince can be used for systems requiring adaptive time-stepping"
+ * (PAPER.md:64; :488 lists adaptive Runge-Kutta as future work) is all the paper says; the rules are DESIGN.md reading Q20:
+ * seven-stage 5(4) pair of Dormand & Prince (1980) with FSAL; error norm err = max over cells, components, reservoirs and
+ * realisations of |E| / (atol + rtol max(|u|, |u_new|)); accept iff err <= 1 (or the proposal is already h_min); next step
+ * h_used * q/16 with q = floor(16 clamp(0.9 err^(-1/5), 1/4, 4)), clamped to [h_min, h_max]; the step that would pass t_end is
+ * clipped to land on it.  One step size for the whole batch.  The whole loop -- stages, error reduction, accept / reject,
+ * step-size control, termination -- runs on the device (a CUDA-graph WHILE node): the call is asynchronous and enqueues one
+ * graph launch.  The adaptive integrator keeps its own clock t (double), starting at 0; phx_set_time moves it.  The drive
+ * phase uses that clock.  UNSUPPORTED: handle created without PHX_INT_DP54, or with noise (a Wiener increment cannot be
+ * re-drawn for a rejected step).  INVALID_ARG: NULL, negative tolerances, atol + rtol == 0, h_min <= 0, h_max < h_min. */
+typedef struct {
+    double atol, rtol;         /* error norm */
+    double h_init;             /* first step size tried when no proposal is pending */
+    double h_min, h_max;       /* clamp of the step size */
+    int64_t max_attempts;      /* at most this many attempts (accepted or rejected) in this call */
+} phx_adaptive;
+
+typedef struct {
+    double t;                  /* time reached */
+    double h_next;             /* step size the next attempt will propose */
+    int64_t n_accept, n_reject;/* totals since creation / phx_set_time */
+    int64_t attempts;          /* attempts of the last call */
+    double err_last;           /* error norm of the last attempt */
+} phx_adaptive_state;
+
+phx_status phx_step_adaptive(phx_grid* g, double t_end, const phx_adaptive* ctl);
+
+/* Synchronises and reads the integrator state back; if the log pointers are non-NULL also the record of every attempt of the
+ * last call (accept flag, q, step used, error norm; at most log_cap records, *n_log receives the number written). */
+phx_status phx_get_adaptive_state(phx_grid* g, phx_adaptive_state* out, int32_t* log_accept, int32_t* log_q, double* log_h,
+                                  double* log_err, int64_t log_cap, int64_t* n_log);
+
+/* Sets the adaptive integrator's clock and pending proposal (h_next <= 0: none); zeroes its counters.  Synchronises. */
+phx_status phx_set_time(phx_grid* g, double t, double h_next);
 
 /* Step counter = number of completed steps.  phx_set_step synchronises. */
 phx_status phx_get_step(const phx_grid* g, uint64_t* step);

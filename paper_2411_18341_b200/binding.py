@@ -25,8 +25,11 @@ PHX_NCOEF = 18
 MODELS = {"scalar": PHX_SCALAR, "reservoir": PHX_RESERVOIR, "spinor": PHX_SPINOR, "spinor_reservoir": PHX_SPINOR_RESERVOIR}
 PRECS = {"c32": PHX_C32, "c64": PHX_C64}
 FIELDS = {"psi_p": PHX_PSI, "psi_m": PHX_PSI_MINUS, "n_p": PHX_N, "n_m": PHX_N_MINUS}
+PHX_INT_RK4, PHX_INT_DP54 = 0, 1
+INTEGRATORS = {"rk4": PHX_INT_RK4, "dp54": PHX_INT_DP54}
 EXPORTS = ("phx_workspace_bytes", "phx_create_grid", "phx_set_params", "phx_set_potential_pump", "phx_set_drive",
-           "phx_set_field", "phx_read_field", "phx_step_rk4", "phx_get_step", "phx_set_step",
+           "phx_set_field", "phx_read_field", "phx_step_rk4", "phx_step_adaptive", "phx_get_adaptive_state", "phx_set_time",
+           "phx_get_step", "phx_set_step",
            "phx_ensemble_mean_density", "phx_get_coeffs", "phx_debug_noise_u32", "phx_select_variant",
            "phx_get_variant", "phx_get_launch_count", "phx_set_tuning", "phx_sync", "phx_last_error",
            "phx_destroy_grid")
@@ -35,13 +38,23 @@ EXPORTS = ("phx_workspace_bytes", "phx_create_grid", "phx_set_params", "phx_set_
 class phx_grid_desc(C.Structure):
     _fields_ = [("nx", C.c_int32), ("ny", C.c_int32), ("batch", C.c_int32), ("dx", C.c_double), ("dy", C.c_double),
                 ("prec", C.c_int32), ("model", C.c_int32), ("noise", C.c_int32), ("bc_x", C.c_int32),
-                ("bc_y", C.c_int32), ("workspace", C.c_void_p), ("workspace_bytes", C.c_size_t),
+                ("bc_y", C.c_int32), ("integrator", C.c_int32), ("workspace", C.c_void_p), ("workspace_bytes", C.c_size_t),
                 ("stream", C.c_void_p)]
 
 
 class phx_params(C.Structure):
     _fields_ = [(k, C.c_double) for k in ("hbar", "m", "g", "g_x", "g_r", "R", "gamma_c", "gamma_r", "beta", "dt",
                                           "noise_scale", "density_offset", "omega")] + [("seed", C.c_uint32)]
+
+
+class phx_adaptive(C.Structure):
+    _fields_ = [("atol", C.c_double), ("rtol", C.c_double), ("h_init", C.c_double), ("h_min", C.c_double),
+                ("h_max", C.c_double), ("max_attempts", C.c_int64)]
+
+
+class phx_adaptive_state(C.Structure):
+    _fields_ = [("t", C.c_double), ("h_next", C.c_double), ("n_accept", C.c_int64), ("n_reject", C.c_int64),
+                ("attempts", C.c_int64), ("err_last", C.c_double)]
 
 
 class PhxError(RuntimeError):
@@ -67,6 +80,8 @@ def lib():
             "phx_create_grid": [vp, vp], "phx_set_params": [vp, vp], "phx_set_potential_pump": [vp, vp, vp, i32],
             "phx_set_drive": [vp, vp, i32], "phx_set_field": [vp, i32, vp, i32], "phx_read_field": [vp, i32, vp, i32],
             "phx_step_rk4": [vp, i64], "phx_get_step": [vp, vp], "phx_set_step": [vp, u64],
+            "phx_step_adaptive": [vp, C.c_double, vp], "phx_get_adaptive_state": [vp, vp, vp, vp, vp, vp, i64, vp],
+            "phx_set_time": [vp, C.c_double, C.c_double],
             "phx_ensemble_mean_density": [vp, i32, vp, i32], "phx_get_coeffs": [vp, vp, i32],
             "phx_debug_noise_u32": [vp, u64, vp, i32], "phx_select_variant": [vp, i32], "phx_get_variant": [vp, vp],
             "phx_get_launch_count": [vp, vp], "phx_set_tuning": [vp, C.c_char_p, i32], "phx_sync": [vp],
@@ -113,7 +128,7 @@ class Grid:
     """One phx_grid handle plus the torch tensor that backs its workspace.  Method names mirror the C ABI."""
 
     def __init__(self, nx, ny, dx, dy, model="scalar", prec="c32", batch=1, noise=False, bc=(0, 0), stream=None,
-                 device="cuda:0"):
+                 device="cuda:0", integrator="rk4"):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("libphx needs a CUDA device (no CPU fallback)")
@@ -122,7 +137,7 @@ class Grid:
         self.cdtype = np.complex64 if prec == "c32" else np.complex128
         self.rdtype = np.float32 if prec == "c32" else np.float64
         self.desc = phx_grid_desc(self.nx, self.ny, self.batch, float(dx), float(dy), PRECS[prec], MODELS[model],
-                                  int(bool(noise)), int(bc[0]), int(bc[1]), None, 0, None)
+                                  int(bool(noise)), int(bc[0]), int(bc[1]), INTEGRATORS[integrator], None, 0, None)
         nbytes = self._lib.phx_workspace_bytes(C.byref(self.desc))
         if nbytes == 0:
             raise PhxError(PHX_ERR_INVALID_ARG, "invalid grid descriptor")
@@ -192,6 +207,25 @@ class Grid:
 
     def step_rk4(self, n_steps=1):
         return self._check(self._lib.phx_step_rk4(self._h, int(n_steps)))
+
+    def step_adaptive(self, t_end, atol, rtol, h_init, h_min=1e-12, h_max=1e30, max_attempts=1 << 40):
+        ctl = phx_adaptive(float(atol), float(rtol), float(h_init), float(h_min), float(h_max), int(max_attempts))
+        return self._check(self._lib.phx_step_adaptive(self._h, float(t_end), C.byref(ctl)))
+
+    def get_adaptive_state(self, log_cap=1 << 16):
+        """Integrator state and the attempt log of the last phx_step_adaptive call (synchronises)."""
+        st = phx_adaptive_state()
+        acc, q = np.zeros(log_cap, np.int32), np.zeros(log_cap, np.int32)
+        h, err = np.zeros(log_cap), np.zeros(log_cap)
+        n = C.c_int64(0)
+        self._check(self._lib.phx_get_adaptive_state(self._h, C.byref(st), acc.ctypes.data, q.ctypes.data, h.ctypes.data,
+                                                     err.ctypes.data, log_cap, C.byref(n)))
+        k = n.value
+        return {"t": st.t, "h_next": st.h_next, "n_accept": st.n_accept, "n_reject": st.n_reject, "attempts": st.attempts,
+                "err_last": st.err_last, "accept": acc[:k], "q": q[:k], "h": h[:k], "err": err[:k]}
+
+    def set_time(self, t, h_next=0.0):
+        return self._check(self._lib.phx_set_time(self._h, float(t), float(h_next)))
 
     def get_step(self):
         v = C.c_uint64()

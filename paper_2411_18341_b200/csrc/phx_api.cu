@@ -4,11 +4,13 @@
 #include "../../include/phx.h"
 
 #include <cmath>
+#include <cstddef>
 #include <cstdio>
 #include <cstring>
 #include <new>
 #include <string>
 
+#include "phx_adaptive.h"
 #include "phx_launch.h"
 #include "phx_stage.cuh"
 #include "phx_step.cuh"
@@ -22,6 +24,7 @@ inline size_t align_up(size_t v) { return (v + ALIGN - 1) / ALIGN * ALIGN; }
 
 struct Layout {
     size_t psi[2], ya[2], yb[2], acc[2], n[2], na[2], nb[2], nacc[2], V, P, E, step, total;
+    size_t K[7][2], Kn[7][2], dpctl, dplog;   // adaptive integrator (PHX_INT_DP54 only)
     size_t scratch_bytes;   // yb[0], acc[0] are contiguous and dead between steps in every variant: scratch
 };
 
@@ -33,6 +36,7 @@ bool desc_ok(const phx_grid_desc* d) {
     if (d->model < PHX_SCALAR || d->model > PHX_SPINOR_RESERVOIR) return false;
     if ((d->bc_x != 0 && d->bc_x != 1) || (d->bc_y != 0 && d->bc_y != 1)) return false;
     if (d->noise != 0 && d->noise != 1) return false;
+    if (d->integrator != PHX_INT_RK4 && d->integrator != PHX_INT_DP54) return false;
     if ((size_t)d->nx * (size_t)d->ny > 0xffffffffull) return false;   // the noise counter holds the cell index in 32 bits
     return true;
 }
@@ -64,6 +68,15 @@ Layout make_layout(const phx_grid_desc* d) {
     L.P = take(plane * rb);
     L.E = take(plane * cb);
     L.step = take(ALIGN);
+    if (d->integrator == PHX_INT_DP54) {
+        for (int q = 0; q < 7; ++q)
+            for (int s = 0; s < nc; ++s) {
+                L.K[q][s] = take(cells * cb);
+                if (res) L.Kn[q][s] = take(cells * rb);
+            }
+        L.dpctl = take(sizeof(DpCtl));
+        L.dplog = take((size_t)DP_LOG_CAP * (2 * sizeof(int) + 2 * sizeof(double)));
+    }
     L.total = off;
     return L;
 }
@@ -91,6 +104,7 @@ struct phx_grid {
     int step_bulk;          // variant STEP fetch path: -1 automatic, 0 register loads, 1 bulk copies into a shared-memory ring
     int async_host;         // 1: host copies of set_field / read_field do not synchronise (pinned buffers, caller syncs)
     cudaGraphExec_t g1[2], gN;  // one step from parity 0 / 1; graph_steps steps from parity 0
+    cudaGraphExec_t gdp;        // adaptive integrator: setup -> WHILE { seven stages, control } -> finalize
     bool graphs_valid;
     int n_sm;
     size_t l2_bytes;        // L2 capacity of the device
@@ -154,6 +168,8 @@ void drop_graphs(phx_grid* g) {
     }
     if (g->gN) cudaGraphExecDestroy(g->gN);
     g->gN = nullptr;
+    if (g->gdp) cudaGraphExecDestroy(g->gdp);
+    g->gdp = nullptr;
     g->graphs_valid = false;
 }
 
@@ -497,6 +513,106 @@ phx_status copy_out(phx_grid* g, void* dst, const void* src, size_t bytes, phx_m
     return PHX_OK;
 }
 
+// ---- adaptive Dormand-Prince 5(4) (phx_adaptive.cu) --------------------------------------------------------------------------
+DpCtl* dp_ctl(phx_grid* g) { return (DpCtl*)(g->ws + g->L.dpctl); }
+
+template <typename T>
+void fill_dp_args(phx_grid* g, DpArgs<T>& a) {
+    using C = typename Cx<T>::type;
+    std::memset(&a, 0, sizeof(a));
+    fill_geo_coef<T>(g, a.geo, a.k);
+    const int nc = model_spinor(g->d.model) ? 2 : 1;
+    const bool res = model_reservoir(g->d.model);
+    for (int s = 0; s < nc; ++s) {
+        a.S[0][s] = (C*)(g->ws + g->L.psi[s]);
+        a.S[1][s] = (C*)(g->ws + g->L.acc[s]);
+        a.Y[0][s] = (C*)(g->ws + g->L.ya[s]);
+        a.Y[1][s] = (C*)(g->ws + g->L.yb[s]);
+        for (int q = 0; q < 7; ++q) a.K[q][s] = (C*)(g->ws + g->L.K[q][s]);
+        if (res) {
+            a.Sn[0][s] = (T*)(g->ws + g->L.n[s]);
+            a.Sn[1][s] = (T*)(g->ws + g->L.nacc[s]);
+            a.Yn[0][s] = (T*)(g->ws + g->L.na[s]);
+            a.Yn[1][s] = (T*)(g->ws + g->L.nb[s]);
+            for (int q = 0; q < 7; ++q) a.Kn[q][s] = (T*)(g->ws + g->L.Kn[q][s]);
+        }
+    }
+    a.V = g->hasV ? (const T*)(g->ws + g->L.V) : nullptr;
+    a.P = g->hasP ? (const T*)(g->ws + g->L.P) : nullptr;
+    a.E = g->hasE ? (const C*)(g->ws + g->L.E) : nullptr;
+    a.ctl = dp_ctl(g);
+    // Dormand & Prince, J. Comput. Appl. Math. 6 (1980) 19: each coefficient a double quotient, rounded once to T
+    const double A[7][7] = {
+        {0, 0, 0, 0, 0, 0, 0},
+        {1.0 / 5.0, 0, 0, 0, 0, 0, 0},
+        {3.0 / 40.0, 9.0 / 40.0, 0, 0, 0, 0, 0},
+        {44.0 / 45.0, -56.0 / 15.0, 32.0 / 9.0, 0, 0, 0, 0},
+        {19372.0 / 6561.0, -25360.0 / 2187.0, 64448.0 / 6561.0, -212.0 / 729.0, 0, 0, 0},
+        {9017.0 / 3168.0, -355.0 / 33.0, 46732.0 / 5247.0, 49.0 / 176.0, -5103.0 / 18656.0, 0, 0},
+        {35.0 / 384.0, 0.0, 500.0 / 1113.0, 125.0 / 192.0, -2187.0 / 6784.0, 11.0 / 84.0, 0}};
+    const double BS[7] = {5179.0 / 57600.0, 0.0, 7571.0 / 16695.0, 393.0 / 640.0, -92097.0 / 339200.0, 187.0 / 2100.0, 1.0 / 40.0};
+    const double Cn[7] = {0.0, 1.0 / 5.0, 3.0 / 10.0, 4.0 / 5.0, 8.0 / 9.0, 1.0, 1.0};
+    for (int s = 0; s < 7; ++s) {
+        a.c[s] = (T)Cn[s];
+        a.e[s] = (T)(A[6][s] - BS[s]);
+        for (int q = 0; q < 7; ++q) a.a[s][q] = (T)A[s][q];
+    }
+}
+
+// Builds the graph  setup -> WHILE { stage 1..7, control } -> finalize  once per handle (it depends on pointers and geometry
+// only; tolerances and t_end travel through the device control block).
+template <typename T>
+cudaError_t build_dp_graph(phx_grid* g) {
+    DpArgs<T> a;
+    fill_dp_args<T>(g, a);
+    const int prec32 = g->d.prec == PHX_C32;
+    cudaGraph_t graph = nullptr;
+    cudaError_t e = cudaGraphCreate(&graph, 0);
+    if (e != cudaSuccess) return e;
+    auto bail = [&](cudaError_t err) { cudaGraphDestroy(graph); return err; };
+    cudaGraphConditionalHandle handle;
+    e = cudaGraphConditionalHandleCreate(&handle, graph, 0, 0);
+    if (e != cudaSuccess) return bail(e);
+    // (1) setup kernel
+    e = cudaStreamBeginCaptureToGraph(g->cap_stream, graph, nullptr, nullptr, 0, cudaStreamCaptureModeThreadLocal);
+    if (e != cudaSuccess) return bail(e);
+    cudaError_t le = dp_launch_setup(a.ctl, (unsigned long long)handle, prec32, g->cap_stream);
+    e = cudaStreamEndCapture(g->cap_stream, &graph);
+    if (le != cudaSuccess) return bail(le);
+    if (e != cudaSuccess) return bail(e);
+    cudaGraphNode_t setup_node = nullptr;
+    size_t nn = 1;
+    e = cudaGraphGetNodes(graph, &setup_node, &nn);
+    if (e != cudaSuccess || nn != 1) return bail(e != cudaSuccess ? e : cudaErrorUnknown);
+    // (2) the WHILE node
+    cudaGraphNodeParams cp = {cudaGraphNodeTypeConditional};
+    cp.type = cudaGraphNodeTypeConditional;
+    cp.conditional.handle = handle;
+    cp.conditional.type = cudaGraphCondTypeWhile;
+    cp.conditional.size = 1;
+    cudaGraphNode_t while_node = nullptr;
+    e = cudaGraphAddNode(&while_node, graph, &setup_node, 1, &cp);
+    if (e != cudaSuccess) return bail(e);
+    cudaGraph_t body = cp.conditional.phGraph_out[0];
+    e = cudaStreamBeginCaptureToGraph(g->cap_stream, body, nullptr, nullptr, 0, cudaStreamCaptureModeThreadLocal);
+    if (e != cudaSuccess) return bail(e);
+    le = dp_launch_attempt<T>(a, g->d.model, g->cap_stream);
+    if (le == cudaSuccess) le = dp_launch_control(a.ctl, (unsigned long long)handle, prec32, DP_LOG_CAP, g->cap_stream);
+    e = cudaStreamEndCapture(g->cap_stream, &body);
+    if (le != cudaSuccess) return bail(le);
+    if (e != cudaSuccess) return bail(e);
+    // (3) finalize, after the loop
+    e = cudaStreamBeginCaptureToGraph(g->cap_stream, graph, &while_node, nullptr, 1, cudaStreamCaptureModeThreadLocal);
+    if (e != cudaSuccess) return bail(e);
+    le = dp_launch_finalize<T>(a, g->d.model, g->n_sm, g->cap_stream);
+    e = cudaStreamEndCapture(g->cap_stream, &graph);
+    if (le != cudaSuccess) return bail(le);
+    if (e != cudaSuccess) return bail(e);
+    e = cudaGraphInstantiate(&g->gdp, graph, 0);
+    cudaGraphDestroy(graph);
+    return e;
+}
+
 }  // namespace
 
 extern "C" {
@@ -542,6 +658,7 @@ phx_status phx_create_grid(phx_grid** out, const phx_grid_desc* desc) {
     g->vec = (desc->prec == PHX_C32 && desc->nx % 2 == 0) ? 2 : 1;
     g->graph_steps = g->gsteps = 8;
     g->g1[0] = g->g1[1] = g->gN = nullptr;
+    g->gdp = nullptr;
     g->graphs_valid = false;
     g->parity = 0;
     g->step_ly = g->step_vec = 0;
@@ -556,6 +673,22 @@ phx_status phx_create_grid(phx_grid** out, const phx_grid_desc* desc) {
     if (cudaStreamCreateWithFlags(&g->cap_stream, cudaStreamNonBlocking) != cudaSuccess) { delete g; return PHX_ERR_CUDA; }
     // zero the state, the static fields and the step counter
     if (cudaMemsetAsync(g->ws, 0, L.total, g->stream) != cudaSuccess) { cudaStreamDestroy(g->cap_stream); delete g; return PHX_ERR_CUDA; }
+    if (desc->integrator == PHX_INT_DP54) {
+        // the control block is all zeros (t = 0, no proposal pending); its log arrays follow it in the workspace
+        DpCtl c;
+        std::memset(&c, 0, sizeof(c));
+        char* lg = g->ws + L.dplog;
+        c.log_accept = (int*)lg;
+        c.log_q = (int*)(lg + (size_t)DP_LOG_CAP * sizeof(int));
+        c.log_h = (double*)(lg + (size_t)DP_LOG_CAP * 2 * sizeof(int));
+        c.log_err = (double*)(lg + (size_t)DP_LOG_CAP * (2 * sizeof(int) + sizeof(double)));
+        if (cudaMemcpyAsync(g->ws + L.dpctl, &c, sizeof(c), cudaMemcpyHostToDevice, g->stream) != cudaSuccess ||
+            cudaStreamSynchronize(g->stream) != cudaSuccess) {
+            cudaStreamDestroy(g->cap_stream);
+            delete g;
+            return PHX_ERR_CUDA;
+        }
+    }
     *out = g;
     return PHX_OK;
 }
@@ -685,6 +818,74 @@ phx_status phx_step_rk4(phx_grid* g, int64_t n_steps) {
     }
     g->step_host += (uint64_t)n_steps;
     g->launches += (uint64_t)n_steps * kernels_per_step(g);
+    return PHX_OK;
+}
+
+phx_status phx_step_adaptive(phx_grid* g, double t_end, const phx_adaptive* ctl) {
+    if (!g || !ctl) return PHX_ERR_INVALID_ARG;
+    if (g->sticky != cudaSuccess) return PHX_ERR_CUDA;
+    if (!g->has_params) return fail(g, PHX_ERR_BAD_STATE, "phx_step_adaptive: call phx_set_params first");
+    if (g->d.integrator != PHX_INT_DP54) return fail(g, PHX_ERR_UNSUPPORTED, "phx_step_adaptive: create the grid with integrator = PHX_INT_DP54");
+    if (g->d.noise) return fail(g, PHX_ERR_UNSUPPORTED, "phx_step_adaptive: not with noise (a Wiener increment cannot be re-drawn for a rejected step)");
+    if (!(ctl->atol >= 0) || !(ctl->rtol >= 0) || !(ctl->atol + ctl->rtol > 0) || !(ctl->h_min > 0) || !(ctl->h_max >= ctl->h_min) ||
+        !(ctl->h_init > 0) || !std::isfinite(t_end) || ctl->max_attempts < 0)
+        return fail(g, PHX_ERR_INVALID_ARG, "phx_step_adaptive: bad tolerances or step-size bounds");
+    // the integrator works on psi / n (and acc / nacc, ya / yb as scratch): bring the state home from the fused step's ping-pong
+    { phx_status s = normalise_state(g); if (s) return s; }
+    if (!g->gdp) {
+        PHX_CUDA(g, g->d.prec == PHX_C64 ? build_dp_graph<double>(g) : build_dp_graph<float>(g));
+    }
+    // call parameters -> head of the device control block (t_end .. max_attempts are its first members)
+    struct { double t_end, atol, rtol, h_init, h_min, h_max; long long max_attempts; } head = {
+        t_end, ctl->atol, ctl->rtol, ctl->h_init, ctl->h_min, ctl->h_max, (long long)ctl->max_attempts};
+    static_assert(offsetof(DpCtl, t) == sizeof(head), "DpCtl head layout");
+    PHX_CUDA(g, cudaMemcpyAsync(g->ws + g->L.dpctl, &head, sizeof(head), cudaMemcpyHostToDevice, g->stream));
+    PHX_CUDA(g, cudaStreamSynchronize(g->stream));   // (`head` is a stack variable: the staged copy must have left it)
+    PHX_CUDA(g, cudaGraphLaunch(g->gdp, g->stream));
+    g->launches += 1;                                 // (graph launches; the kernels inside are counted by phx_get_adaptive_state)
+    return PHX_OK;
+}
+
+phx_status phx_get_adaptive_state(phx_grid* g, phx_adaptive_state* out, int32_t* log_accept, int32_t* log_q, double* log_h,
+                                  double* log_err, int64_t log_cap, int64_t* n_log) {
+    if (!g || !out) return PHX_ERR_INVALID_ARG;
+    if (g->sticky != cudaSuccess) return PHX_ERR_CUDA;
+    if (g->d.integrator != PHX_INT_DP54) return fail(g, PHX_ERR_UNSUPPORTED, "phx_get_adaptive_state: not an adaptive grid");
+    DpCtl c;
+    PHX_CUDA(g, cudaMemcpyAsync(&c, g->ws + g->L.dpctl, sizeof(c), cudaMemcpyDeviceToHost, g->stream));
+    PHX_CUDA(g, cudaStreamSynchronize(g->stream));
+    out->t = c.t;
+    out->h_next = c.h;
+    out->n_accept = c.n_accept;
+    out->n_reject = c.n_reject;
+    out->attempts = c.attempts;
+    out->err_last = c.err_last;
+    int64_t n = c.log_count < DP_LOG_CAP ? c.log_count : DP_LOG_CAP;
+    if (n > log_cap) n = log_cap;
+    if (n < 0) n = 0;
+    if (n_log) *n_log = n;
+    if (n > 0) {
+        if (log_accept) PHX_CUDA(g, cudaMemcpy(log_accept, c.log_accept, n * sizeof(int), cudaMemcpyDeviceToHost));
+        if (log_q) PHX_CUDA(g, cudaMemcpy(log_q, c.log_q, n * sizeof(int), cudaMemcpyDeviceToHost));
+        if (log_h) PHX_CUDA(g, cudaMemcpy(log_h, c.log_h, n * sizeof(double), cudaMemcpyDeviceToHost));
+        if (log_err) PHX_CUDA(g, cudaMemcpy(log_err, c.log_err, n * sizeof(double), cudaMemcpyDeviceToHost));
+    }
+    return PHX_OK;
+}
+
+phx_status phx_set_time(phx_grid* g, double t, double h_next) {
+    if (!g || !std::isfinite(t)) return PHX_ERR_INVALID_ARG;
+    if (g->sticky != cudaSuccess) return PHX_ERR_CUDA;
+    if (g->d.integrator != PHX_INT_DP54) return fail(g, PHX_ERR_UNSUPPORTED, "phx_set_time: not an adaptive grid");
+    DpCtl c;
+    PHX_CUDA(g, cudaMemcpyAsync(&c, g->ws + g->L.dpctl, sizeof(c), cudaMemcpyDeviceToHost, g->stream));
+    PHX_CUDA(g, cudaStreamSynchronize(g->stream));
+    c.t = t;
+    c.h = h_next > 0 ? h_next : 0.0;
+    c.n_accept = c.n_reject = 0;
+    c.k1_valid = 0;
+    PHX_CUDA(g, cudaMemcpyAsync(g->ws + g->L.dpctl, &c, sizeof(c), cudaMemcpyHostToDevice, g->stream));
+    PHX_CUDA(g, cudaStreamSynchronize(g->stream));
     return PHX_OK;
 }
 

@@ -20,10 +20,11 @@ using namespace phx;
 namespace {
 
 constexpr size_t ALIGN = 256;
+constexpr size_t FLAG_BYTES = 64 * 1024;   // progress counters of the persistent fused step: one uint32 per tile (warp)
 inline size_t align_up(size_t v) { return (v + ALIGN - 1) / ALIGN * ALIGN; }
 
 struct Layout {
-    size_t psi[2], ya[2], yb[2], acc[2], n[2], na[2], nb[2], nacc[2], V, P, E, step, total;
+    size_t psi[2], ya[2], yb[2], acc[2], n[2], na[2], nb[2], nacc[2], V, P, E, step, flags, total;
     size_t K[7][2], Kn[7][2], dpctl, dplog;   // adaptive integrator (PHX_INT_DP54 only)
     size_t scratch_bytes;   // yb[0], acc[0] are contiguous and dead between steps in every variant: scratch
 };
@@ -68,6 +69,7 @@ Layout make_layout(const phx_grid_desc* d) {
     L.P = take(plane * rb);
     L.E = take(plane * cb);
     L.step = take(ALIGN);
+    L.flags = take(FLAG_BYTES);
     if (d->integrator == PHX_INT_DP54) {
         for (int q = 0; q < 7; ++q)
             for (int s = 0; s < nc; ++s) {
@@ -102,6 +104,9 @@ struct phx_grid {
     int step_ly, step_vec;  // variant STEP geometry (0 = automatic)
     int step_warps;         // variant STEP warps per CTA (0 = automatic)
     int step_bulk;          // variant STEP fetch path: -1 automatic, 0 register loads, 1 bulk copies into a shared-memory ring
+    int step_xch;           // variant STEP exchanging strips (the warps of a CTA tile the whole row): -1 automatic, 0 off
+    int step_persist;       // variant STEP persistent launch (all steps of a call in one cooperative launch): -1 automatic, 0 off, 1 on
+    bool persist_failed;    // the cooperative launch was refused for the current plan (tiles not all resident): graphs instead
     int async_host;         // 1: host copies of set_field / read_field do not synchronise (pinned buffers, caller syncs)
     cudaGraphExec_t g1[2], gN;  // one step from parity 0 / 1; graph_steps steps from parity 0
     cudaGraphExec_t gdp;        // adaptive integrator: setup -> WHILE { seven stages, control } -> finalize
@@ -171,6 +176,7 @@ void drop_graphs(phx_grid* g) {
     if (g->gdp) cudaGraphExecDestroy(g->gdp);
     g->gdp = nullptr;
     g->graphs_valid = false;
+    g->persist_failed = false;      // (the launch plan may have changed)
 }
 
 template <typename T>
@@ -298,13 +304,7 @@ int step_strips(const phx_grid* g, int vec) { return (g->d.nx + 32 * vec - 9) / 
 // Warps per CTA: the warps of a CTA own adjacent strips and are otherwise independent.  Two per CTA measured 4 % faster
 // than one on the 16384^2 spinor and equal on the 4096^2 reservoir grid; but a row with an odd number of strips leaves the
 // last CTA's second warp idle: 1 of 6 warp slots on the 256-wide grids of cfg5 (5 strips: 91 against 75 Gcell*step/s with
-// one warp per CTA), 1 of 36 at 4096^2 scalar fp32 (+1.4 %).  One warp per CTA when more than 2 % of the slots would idle.
-int step_warps(const phx_grid* g, int vec) {
-    if (g->step_warps) return g->step_warps;
-    const int strips = step_strips(g, vec);
-    return (strips % PHX_STEP_WARPS != 0 && strips < 50) ? 1 : PHX_STEP_WARPS;
-}
-
+// one warp per CTA), 1 of 36 at 4096^2 scalar fp32.  The launch plan (step_plan below) compares the two.
 // Bytes one step of variant STEP touches per cell (state in and out, V, P, E).
 size_t step_bytes_per_cell(const phx_grid* g) {
     const size_t rb = real_bytes(g);
@@ -317,29 +317,65 @@ size_t step_bytes_per_cell(const phx_grid* g) {
     return b;
 }
 
-// Rows per chunk.  Every CTA costs (ly + 6) row iterations (4 + 4 halo rows and the pipeline fill, less the two rows
-// the prologue fetches) rounded up to the unroll factor of the row loop (5, the ring length).
+// Launch plan: rows per chunk (ly) and warps per CTA (wpc).  A chunk costs ly + 6 row iterations (4 + 4 halo rows and the
+// pipeline fill, less the two rows the prologue fetches); the bulk-copy path runs whole passes of the unrolled row loop.
 //  - Working set beyond L2 (the BASELINE grids from 4096^2 up, cfg5): an iteration waits on DRAM, more resident warps
 //    hide it, and the grid runs in ceil(CTAs / resident CTAs) waves: minimise waves * iterations.
 //  - Working set within half of L2 (1024^2): two warps per scheduler already saturate the FP32 pipe (measured at
 //    1024^2 fp32: 525 cycles per iteration with 1-2 warps per scheduler, 810 with 3, 1250 with 4), so fewer, longer
 //    chunks win: minimise iterations * max(1.75, warps per scheduler) (ly = 19 instead of 9: 113 instead of 80
 //    Gcell*step/s).
-int step_rows_per_chunk(const phx_grid* g, int vec) {
-    if (g->step_ly) return g->step_ly < g->d.ny ? g->step_ly : g->d.ny;
-    const int strips = step_strips(g, vec), wpc = step_warps(g, vec);
+//  One warp per CTA is taken when it is at least 2 % cheaper than two by this count (4096^2 scalar fp32: 35 strips x 33
+//  chunks of 125 rows fill 1155 of 1184 warp slots, 131 iterations; in pairs 18 x 32 CTAs of 128 rows, 134 iterations).
+struct StepPlan { int ly, wpc, vec; bool xch; };
+
+// Exchanging strips (phx_step.cuh, XCH): cells per lane with which the warps of one CTA tile the whole row, or 0.
+// Periodic scalar / reservoir grids without drive whose width is 1 .. PHX_STEP_XWARPS strips of 32 * vec columns.
+// Automatic (step_xch = -1): rows of at most 4 strips of 2 (fp64: 1) cells per lane on work of a million cells or more -- the
+// ensembles of narrow grids, where the recomputed halo columns cost most (cfg5, 5 strips -> 4: 99.9 against 88.5
+// Gcell*step/s; 512 x 64^2: 81.8 against 29.4).  A single small grid is latency-bound and the barrier per iteration costs it
+// (64^2: 4.6 against 4.4 us per step), and 8 warps of 4 cells per lane on a 1024-wide row lose to the independent strips (80
+// against 102-110): those run it only when asked for (step_xch = 1).
+int stepx_vec(const phx_grid* g) {
+    if (g->step_xch == 0) return 0;
+    if (g->d.bc_x || g->d.bc_y || g->hasE || g->d.model > PHX_RESERVOIR) return 0;
+    const bool forced = g->step_xch == 1;
+    if (!forced && plane_cells(g) * g->d.batch < ((size_t)1 << 20)) return 0;
+    for (int vec = 4; vec >= 1; vec >>= 1) {
+        if (g->step_vec && vec != g->step_vec) continue;
+        if (!stepx_has_vec(g->d.prec == PHX_C64, g->d.model, vec)) continue;
+        const int w = 32 * vec;
+        if (g->d.nx % w != 0 || g->d.nx / w > PHX_STEP_XWARPS) continue;
+        if (!forced && (g->d.nx / w > 4 || vec > (g->d.prec == PHX_C64 ? 1 : 2))) continue;
+        return vec;
+    }
+    return 0;
+}
+
+int stepx_occupancy(const phx_grid* g, int vec, int warps) {
+    const bool noise = g->d.noise != 0, iso = step_iso(g);
+    if (g->d.prec == PHX_C32)
+        return g->d.model == 0 ? occupancy_stepx_32_0(noise, iso, vec, warps) : occupancy_stepx_32_1(noise, iso, vec, warps);
+    return g->d.model == 0 ? occupancy_stepx_64_0(noise, iso, vec, warps) : occupancy_stepx_64_1(noise, iso, vec, warps);
+}
+
+double step_plan_cost(const phx_grid* g, int vec, int wpc, int* ly_out, bool xch = false) {
+    const int strips = xch ? wpc : step_strips(g, vec);
     const long ctas_row = (long)((strips + wpc - 1) / wpc) * g->d.batch;
-    const long slots = (long)g->n_sm * step_occupancy(g, vec) * (PHX_STEP_WARPS / wpc);   // resident CTAs of wpc warps
+    const long slots = xch ? (long)g->n_sm * stepx_occupancy(g, vec, wpc)
+                           : (long)g->n_sm * step_occupancy(g, vec) * (PHX_STEP_WARPS / wpc);   // resident CTAs of wpc warps
     const bool in_l2 = plane_cells(g) * g->d.batch * step_bytes_per_cell(g) < g->l2_bytes / 2;
+    const bool whole_passes = xch || step_bulk(g) || !step_early_exit(g->d.prec == PHX_C64, g->d.model, vec);
     double best_cost = -1;
     int best_ly = g->d.ny;
     const int max_chunks = g->d.ny / 4 > 0 ? g->d.ny / 4 : 1;   // (a 64^2 grid: ly = 4, 3.6 instead of 4.9 us per step)
     for (int nch = 1; nch <= max_chunks && nch <= 65535; ++nch) {
-        const int ly = (g->d.ny + nch - 1) / nch;
+        int ly = (g->d.ny + nch - 1) / nch;
+        if (g->step_ly) ly = g->step_ly < g->d.ny ? g->step_ly : g->d.ny;
         const int real_chunks = (g->d.ny + ly - 1) / ly;
         const long ctas = ctas_row * real_chunks;
         const long waves = (ctas + slots - 1) / slots;
-        const long iters = (ly + 6 + PHX_STEP_RING - 1) / PHX_STEP_RING * PHX_STEP_RING;
+        const long iters = whole_passes ? (ly + 6 + PHX_STEP_RING - 1) / PHX_STEP_RING * PHX_STEP_RING : ly + 6;
         double cost = (double)(waves * iters);
         if (in_l2) {
             const long per_sm = ((ctas + waves - 1) / waves + g->n_sm - 1) / g->n_sm;     // CTAs on the fullest SM
@@ -347,13 +383,42 @@ int step_rows_per_chunk(const phx_grid* g, int vec) {
             cost *= per_sched > 1.75 ? (double)per_sched : 1.75;
         }
         if (best_cost < 0 || cost < best_cost) { best_cost = cost; best_ly = ly; }
+        if (g->step_ly) break;
     }
-    return best_ly;
+    *ly_out = best_ly;
+    return best_cost;
+}
+
+StepPlan step_plan(const phx_grid* g) {
+    StepPlan p;
+    p.xch = false;
+    if (const int xv = stepx_vec(g)) {
+        p.xch = true;
+        p.vec = xv;
+        p.wpc = g->d.nx / (32 * xv);
+        step_plan_cost(g, xv, p.wpc, &p.ly, true);
+        return p;
+    }
+    const int vec = p.vec = step_vec(g);
+    if (g->step_warps) {
+        p.wpc = g->step_warps;
+        step_plan_cost(g, vec, p.wpc, &p.ly);
+        return p;
+    }
+    int ly2 = 0, ly1 = 0;
+    const double c2 = step_plan_cost(g, vec, PHX_STEP_WARPS, &ly2), c1 = step_plan_cost(g, vec, 1, &ly1);
+    const int strips = step_strips(g, vec);
+    const bool idle_warp = strips % PHX_STEP_WARPS != 0 && strips < 50;   // pairs would leave more than 2 % of the warp slots idle
+    if (c1 * 1.02 < c2 || (idle_warp && c1 <= c2 * 1.02)) { p.wpc = 1; p.ly = ly1; }
+    else { p.wpc = PHX_STEP_WARPS; p.ly = ly2; }
+    return p;
 }
 
 // One RK4 step of variant STEP: a single kernel that reads the state of parity p and writes parity 1-p.
+// n_persist > 0: the PERSISTENT launch instead -- n_persist steps in one cooperative launch (phx_step.cuh, PERS), the state
+// ends in parity p ^ (n_persist & 1); cudaErrorCooperativeLaunchTooLarge when the tiles are not all resident.
 template <typename T>
-cudaError_t enqueue_step_fused(phx_grid* g, cudaStream_t st, int parity) {
+cudaError_t enqueue_step_fused(phx_grid* g, cudaStream_t st, int parity, int n_persist = 0) {
     using C = typename Cx<T>::type;
     StepArgs<T> a;
     std::memset(&a, 0, sizeof(a));
@@ -379,13 +444,50 @@ cudaError_t enqueue_step_fused(phx_grid* g, cudaStream_t st, int parity) {
     a.step_in = slots + parity;
     a.step_out = slots + (1 - parity);
     a.seed = g->prm.seed;
-    const int vec = step_vec(g);
-    a.strips = step_strips(g, vec);
-    a.wpc = step_warps(g, vec);
-    a.ly = step_rows_per_chunk(g, vec);
+    const StepPlan plan = step_plan(g);
+    const int vec = plan.vec;
+    a.strips = plan.xch ? plan.wpc : step_strips(g, vec);
+    a.wpc = plan.wpc;
+    a.ly = plan.ly;
     const dim3 grid((a.strips + a.wpc - 1) / a.wpc, (g->d.ny + a.ly - 1) / a.ly, g->d.batch);
     if (grid.y > 65535u) return cudaErrorInvalidConfiguration;
     const bool noise = g->d.noise != 0, zbc = g->d.bc_x || g->d.bc_y, iso = step_iso(g), bulk = step_bulk(g);
+    if (n_persist > 0) {
+        const size_t tiles = (size_t)a.strips * grid.y * grid.z;
+        if (zbc || bulk || g->hasE || tiles * sizeof(uint32_t) > FLAG_BYTES) return cudaErrorCooperativeLaunchTooLarge;
+        a.n_steps = n_persist;
+        a.step0 = g->step_host;
+        a.flags = (uint32_t*)(g->ws + g->L.flags);
+        cudaError_t e = cudaMemsetAsync(a.flags, 0, tiles * sizeof(uint32_t), st);
+        if (e != cudaSuccess) return e;
+        if (plan.xch) {
+            if constexpr (sizeof(T) == 4)
+                return g->d.model == 0 ? launch_stepxp_32_0(a, noise, iso, vec, grid, st) : launch_stepxp_32_1(a, noise, iso, vec, grid, st);
+            else
+                return g->d.model == 0 ? launch_stepxp_64_0(a, noise, iso, vec, grid, st) : launch_stepxp_64_1(a, noise, iso, vec, grid, st);
+        }
+        if constexpr (sizeof(T) == 4) {
+            switch (g->d.model) {
+                case 0: return launch_stepp_32_0(a, noise, zbc, iso, bulk, vec, grid, st);
+                case 1: return launch_stepp_32_1(a, noise, zbc, iso, bulk, vec, grid, st);
+                case 2: return launch_stepp_32_2(a, noise, zbc, iso, bulk, vec, grid, st);
+                default: return launch_stepp_32_3(a, noise, zbc, iso, bulk, vec, grid, st);
+            }
+        } else {
+            switch (g->d.model) {
+                case 0: return launch_stepp_64_0(a, noise, zbc, iso, bulk, vec, grid, st);
+                case 1: return launch_stepp_64_1(a, noise, zbc, iso, bulk, vec, grid, st);
+                case 2: return launch_stepp_64_2(a, noise, zbc, iso, bulk, vec, grid, st);
+                default: return launch_stepp_64_3(a, noise, zbc, iso, bulk, vec, grid, st);
+            }
+        }
+    }
+    if (plan.xch) {
+        if constexpr (sizeof(T) == 4)
+            return g->d.model == 0 ? launch_stepx_32_0(a, noise, iso, vec, grid, st) : launch_stepx_32_1(a, noise, iso, vec, grid, st);
+        else
+            return g->d.model == 0 ? launch_stepx_64_0(a, noise, iso, vec, grid, st) : launch_stepx_64_1(a, noise, iso, vec, grid, st);
+    }
     if constexpr (sizeof(T) == 4) {
         switch (g->d.model) {
             case 0: return launch_step_32_0(a, noise, zbc, iso, bulk, vec, grid, st);
@@ -401,6 +503,17 @@ cudaError_t enqueue_step_fused(phx_grid* g, cudaStream_t st, int parity) {
             default: return launch_step_64_3(a, noise, zbc, iso, bulk, vec, grid, st);
         }
     }
+}
+
+// The persistent launch of the fused step: periodic grids without drive, and only when asked for (step_persist = 1).  Measured
+// slower than one launch per step replayed from a CUDA graph on every BASELINE workload (same run, Gcell*step/s: 1024^2 fp32
+// 51 against 111, 4096^2 fp32 181 against 211, cfg3 117 against 146, 16384^2 spinor 71 against 82; one 64^2 grid 3.9 against
+// 3.6 us per step): between steps a warp pays a fence, a release store, the neighbours' acquire polls and the refill of its
+// row pipeline, the state has to be read through L2 (ld.global.cg) instead of the non-coherent path, and the step loop costs
+// registers the row loop needs (spills).  DESIGN.md section 5.2.
+bool persist_wanted(const phx_grid* g) {
+    if (g->step_persist != 1 || g->persist_failed) return false;
+    return !(g->d.bc_x || g->d.bc_y || g->hasE || step_bulk(g));
 }
 
 int kernels_per_step(const phx_grid* g) { return g->variant == PHX_VARIANT_STEP ? 1 : 4; }   // (RESIDENT: one per call)
@@ -663,6 +776,9 @@ phx_status phx_create_grid(phx_grid** out, const phx_grid_desc* desc) {
     g->parity = 0;
     g->step_ly = g->step_vec = 0;
     g->step_bulk = -1;
+    g->step_xch = -1;
+    g->step_persist = -1;
+    g->persist_failed = false;
     g->step_warps = 0;
     g->async_host = 0;
     g->n_sm = prop.multiProcessorCount;
@@ -791,8 +907,30 @@ phx_status phx_step_rk4(phx_grid* g, int64_t n_steps) {
         }
         return PHX_OK;
     }
+    if (g->variant == PHX_VARIANT_STEP && n_steps >= 2 && persist_wanted(g)) {
+        int64_t left = n_steps;
+        while (left > 0) {
+            const int chunk = left > (1 << 20) ? (1 << 20) : (int)left;
+            const cudaError_t e = g->d.prec == PHX_C64 ? enqueue_step_fused<double>(g, g->stream, g->parity, chunk)
+                                                       : enqueue_step_fused<float>(g, g->stream, g->parity, chunk);
+            if (e == cudaErrorCooperativeLaunchTooLarge) {      // not all tiles resident: the graphs of single-step launches instead
+                cudaGetLastError();
+                g->persist_failed = true;
+                break;
+            }
+            PHX_CUDA(g, e);
+            g->parity ^= chunk & 1;
+            g->step_host += (uint64_t)chunk;
+            g->launches += 1;
+            left -= chunk;
+        }
+        if (left == 0) return PHX_OK;
+        n_steps = left;
+    }
     if (!g->graphs_valid) {
+        const bool refused = g->persist_failed;
         drop_graphs(g);
+        g->persist_failed = refused;
         PHX_CUDA(g, capture(g, 1, 0, &g->g1[0]));
         if (g->variant == PHX_VARIANT_STEP) PHX_CUDA(g, capture(g, 1, 1, &g->g1[1]));
         // the multi-step graph of the ping-pong variant must return to parity 0: an even number of steps
@@ -995,6 +1133,12 @@ phx_status phx_set_tuning(phx_grid* g, const char* key, int32_t value) {
     } else if (!std::strcmp(key, "step_bulk")) {      // variant STEP fetch path: -1 automatic, 0 register loads, 1 bulk copies
         if (value < -1 || value > 1) return PHX_ERR_INVALID_ARG;
         g->step_bulk = value;
+    } else if (!std::strcmp(key, "step_xch")) {       // variant STEP exchanging strips: -1 automatic (wherever the row fits), 0 off
+        if (value < -1 || value > 1) return PHX_ERR_INVALID_ARG;
+        g->step_xch = value;
+    } else if (!std::strcmp(key, "step_persist")) {   // variant STEP persistent launch: 1 on; -1 (automatic) and 0: off
+        if (value < -1 || value > 1) return PHX_ERR_INVALID_ARG;
+        g->step_persist = value;
     } else if (!std::strcmp(key, "async_host_copies")) {   // 1: phx_set_field / phx_read_field with PHX_HOST do not synchronise
         if (value != 0 && value != 1) return PHX_ERR_INVALID_ARG;
         g->async_host = value;

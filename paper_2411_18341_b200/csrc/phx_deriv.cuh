@@ -47,11 +47,16 @@ struct Diff {
 };
 
 // NINE: the spinor models (all nine points, A, B, D kept).  ISO: dx == dy, so cx == cy and
-// L = cx ((e + w) + (n + s) - 4 c) -- one packed operation fewer, exact factors only.
+// L = cx ((e + w) + (n + s) - 4 c) -- one packed operation fewer, exact factors only.  NINE and ISO: bxx == byy as well
+// (both are beta / (hbar d^2) of the same d), so the TE-TM operator needs only A - B = (e + w) - (n + s), kept in A.
 template <typename T, bool NINE, bool ISO>
 __device__ __forceinline__ void differences(const Coef<T>& k, const Nbhd<T>& nb, Diff<T>& d) {
     if (ISO && !NINE) {
         d.L = mul2s(k.cx, fma2s(T(-4), nb.c, add2(add2(nb.e, nb.w), add2(nb.n, nb.s))));
+    } else if (ISO) {
+        const typename Cx<T>::type ew = add2(nb.e, nb.w), ns = add2(nb.n, nb.s);
+        d.L = mul2s(k.cx, fma2s(T(-4), nb.c, add2(ew, ns)));
+        d.A = sub2(ew, ns);
     } else {
         d.A = fma2s(T(-2), nb.c, add2(nb.e, nb.w));
         d.B = fma2s(T(-2), nb.c, add2(nb.n, nb.s));
@@ -64,7 +69,7 @@ __device__ __forceinline__ void differences(const Coef<T>& k, const Nbhd<T>& nb,
 //   y, own:  this component's value and differences;  yo, oth: the other component's (SPINOR only)
 //   upper:   true for the psi_+ equation (operator (d_x - i d_y)^2 acts on psi_-)
 //   Ed, q:  drive amplitude E(r) of the cell and q = (1/hbar) exp(-i omega t_s) (DRIVE only):  K += -i q E
-template <typename T, bool SPINOR, bool RES, bool DRIVE>
+template <typename T, bool SPINOR, bool RES, bool DRIVE, bool ISO = false>
 __device__ __forceinline__ typename Cx<T>::type deriv(const Coef<T>& k, typename Cx<T>::type y, const Diff<T>& own,
                                                       typename Cx<T>::type yo, const Diff<T>& oth, bool upper, T nres, T V,
                                                       T P, typename Cx<T>::type Ed, typename Cx<T>::type q, T& Kn) {
@@ -80,8 +85,8 @@ __device__ __forceinline__ typename Cx<T>::type deriv(const Coef<T>& k, typename
     // operand, where the packed instruction takes it as a modifier)
     C M = fma2s(-W, y, own.L);
     if (SPINOR) {
-        M = fma2s(-k.bxx, oth.A, M);
-        M = fma2s(k.byy, oth.B, M);
+        M = fma2s(-k.bxx, oth.A, M);                 // (ISO: oth.A holds Dxx - Dyy and bxx == byy)
+        if (!ISO) M = fma2s(k.byy, oth.B, M);
     }
     // -i q E = i (-q_re E) + q_im E: the first part joins M (rotated below), the second K
     if (DRIVE) M = fma2s(-q.x, Ed, M);

@@ -9,12 +9,37 @@
 #define PHX_STEP_WARPS 2
 #endif
 
+// Variant STEP, exchanging strips (phx_step.cuh, XCH): most warps per CTA; the warps of a CTA tile the whole row.
+#ifndef PHX_STEP_XWARPS
+#define PHX_STEP_XWARPS 8
+#endif
+// How the warps of a row wait for each other: 0 = a progress counter per warp, polled (neighbours drift by up to one iteration);
+// 1 = one named barrier per iteration (lockstep, no branch in the row loop).
+// (measured on cfg5, 512 x 256^2 reservoir + noise: barrier 99.9, counters 74.6, no exchange 88.5 Gcell*step/s: the spin loop
+// splits every phase of the row loop into basic blocks)
+#ifndef PHX_XCH_SYNC
+#define PHX_XCH_SYNC 1
+#endif
+
 // Variant STEP: row iterations a fetch leads its first use by, and the ring length / unroll factor of the row loop.
 // (LEAD = 2 costs registers and is slower everywhere: 200.6 against 207.5 Gcell*step/s at 4096^2 fp32, spills in the spinor.)
 #ifndef PHX_STEP_LEAD
 #define PHX_STEP_LEAD 1
 #endif
 #define PHX_STEP_RING (4 + PHX_STEP_LEAD)
+// Leave the unrolled row loop in the middle of its last pass (a chunk of ly rows costs ly + 6 iterations instead of the next
+// multiple of the ring length).  The exit test splits the loop body into one basic block per phase, which costs the other
+// kernels more than the saved iterations give back (same-run A/B: 4096^2 scalar fp32 4 cells per lane 213 against 205
+// Gcell*step/s and 1024^2 scalar fp64 2 cells per lane 70.8 against 64.3 with the exit; cfg3 reservoir 141.6 against 147.6,
+// 1024^2 fp32 101.8 against 110.3, a single 64^2 fp64 grid 5.4 against 3.8 us per step without): taken by those two only.
+#ifndef PHX_STEP_EARLY_EXIT
+#define PHX_STEP_EARLY_EXIT 1
+#endif
+namespace phx {
+constexpr bool step_early_exit(bool prec64, int model, int vec) {
+    return PHX_STEP_EARLY_EXIT && model == 0 && ((!prec64 && vec == 4) || (prec64 && vec == 2));
+}
+}
 // Bulk-copy fetch path of variant STEP: stages of the per-warp shared-memory ring (rows in flight = DEPTH - 1); power of 2.
 #ifndef PHX_STEP_DEPTH
 #define PHX_STEP_DEPTH 8
@@ -47,6 +72,46 @@ template <typename T> struct StepArgs;
 PHX_DECL_STEP(32, float)
 PHX_DECL_STEP(64, double)
 #undef PHX_DECL_STEP
+
+// the persistent launch of the fused step (phx_step_inst.cu compiled with -DPHX_INST_PERS=1): a.n_steps steps in one cooperative
+// launch; periodic boundaries, no drive (zbc and bulk must be false); cudaErrorCooperativeLaunchTooLarge if the grid is not resident
+#define PHX_DECL_STEPP(P, T)                                                                                      \
+    cudaError_t launch_stepp_##P##_0(const StepArgs<T>&, bool noise, bool zbc, bool iso, bool bulk, int vec, dim3 grid, cudaStream_t); \
+    cudaError_t launch_stepp_##P##_1(const StepArgs<T>&, bool noise, bool zbc, bool iso, bool bulk, int vec, dim3 grid, cudaStream_t); \
+    cudaError_t launch_stepp_##P##_2(const StepArgs<T>&, bool noise, bool zbc, bool iso, bool bulk, int vec, dim3 grid, cudaStream_t); \
+    cudaError_t launch_stepp_##P##_3(const StepArgs<T>&, bool noise, bool zbc, bool iso, bool bulk, int vec, dim3 grid, cudaStream_t); \
+    int occupancy_stepp_##P##_0(bool noise, bool zbc, bool iso, bool drive, bool bulk, int vec);                                          \
+    int occupancy_stepp_##P##_1(bool noise, bool zbc, bool iso, bool drive, bool bulk, int vec);                                          \
+    int occupancy_stepp_##P##_2(bool noise, bool zbc, bool iso, bool drive, bool bulk, int vec);                                          \
+    int occupancy_stepp_##P##_3(bool noise, bool zbc, bool iso, bool drive, bool bulk, int vec);
+PHX_DECL_STEPP(32, float)
+PHX_DECL_STEPP(64, double)
+#undef PHX_DECL_STEPP
+
+// phx_stepx_inst.cu: the fused step with exchanging strips (scalar and reservoir models, periodic, no drive).  `vec` must be
+// one the precision and model have (stepx_has_vec); the CTA has a.wpc warps; occupancy = resident CTAs of `warps` warps per SM.
+#define PHX_DECL_STEPX(P, T)                                                                                  \
+    cudaError_t launch_stepx_##P##_0(const StepArgs<T>&, bool noise, bool iso, int vec, dim3 grid, cudaStream_t); \
+    cudaError_t launch_stepx_##P##_1(const StepArgs<T>&, bool noise, bool iso, int vec, dim3 grid, cudaStream_t); \
+    int occupancy_stepx_##P##_0(bool noise, bool iso, int vec, int warps);                                        \
+    int occupancy_stepx_##P##_1(bool noise, bool iso, int vec, int warps);
+PHX_DECL_STEPX(32, float)
+PHX_DECL_STEPX(64, double)
+#undef PHX_DECL_STEPX
+#define PHX_DECL_STEPXP(P, T)                                                                                  \
+    cudaError_t launch_stepxp_##P##_0(const StepArgs<T>&, bool noise, bool iso, int vec, dim3 grid, cudaStream_t); \
+    cudaError_t launch_stepxp_##P##_1(const StepArgs<T>&, bool noise, bool iso, int vec, dim3 grid, cudaStream_t); \
+    int occupancy_stepxp_##P##_0(bool noise, bool iso, int vec, int warps);                                        \
+    int occupancy_stepxp_##P##_1(bool noise, bool iso, int vec, int warps);
+PHX_DECL_STEPXP(32, float)
+PHX_DECL_STEPXP(64, double)
+#undef PHX_DECL_STEPXP
+// cells per lane the exchanging strips are instantiated with: complex fp32 2 (scalar also 4), complex fp64 1 (scalar also 2)
+inline bool stepx_has_vec(int prec64, int model, int vec) {
+    if (model > 1) return false;
+    if (!prec64) return vec == 2 || (vec == 4 && model == 0);
+    return vec == 1 || (vec == 2 && model == 0);
+}
 
 // phx_resident.cu: variant RESIDENT (a small grid on chip for all steps of one launch)
 #ifndef PHX_RESIDENT_THREADS

@@ -18,6 +18,8 @@
 // 14 complex transfers of variant STAGE.  psi(t) and psi(t+dt) are distinct buffers (ping-pong).
 #pragma once
 
+#include <climits>
+
 #include "phx_common.cuh"
 #include "phx_deriv.cuh"
 #include "phx_philox.cuh"
@@ -47,23 +49,30 @@ struct StepArgs {
     int ly;                     // rows per chunk
     int strips;                 // strips per row of the grid
     int wpc;                    // warps per CTA of this launch (1 .. PHX_STEP_WARPS; the warps of a CTA are independent)
+    // persistent launch (template switch PERS): n_steps RK4 steps in ONE cooperative launch
+    int n_steps;
+    uint64_t step0;             // completed steps before this launch (the host's count; the device slots are written at the end)
+    uint32_t* flags;            // [batch][chunks][strips]: steps of this launch the tile has finished (zeroed before the launch)
 };
 
 namespace stepk {
 
-template <int VEC> __device__ __forceinline__ void ldc(const float2* p, float2 (&v)[VEC]) {
+// CG: the array is rewritten by other SMs during the launch (persistent kernel): load through L2 (ld.global.cg), not through
+// the non-coherent path, whose L1 lines may date from two steps ago.
+template <bool CG, typename Q> __device__ __forceinline__ Q ldx(const Q* p) { return CG ? __ldcg(p) : __ldg(p); }
+template <int VEC, bool CG = false> __device__ __forceinline__ void ldc(const float2* p, float2 (&v)[VEC]) {
     if constexpr (VEC % 2 == 0) {
 #pragma unroll
         for (int h = 0; h < VEC / 2; ++h) {
-            const float4 q = __ldg(reinterpret_cast<const float4*>(p) + h);
+            const float4 q = ldx<CG>(reinterpret_cast<const float4*>(p) + h);
             v[2 * h] = make_float2(q.x, q.y);
             v[2 * h + 1] = make_float2(q.z, q.w);
         }
-    } else v[0] = __ldg(p);
+    } else v[0] = ldx<CG>(p);
 }
-template <int VEC> __device__ __forceinline__ void ldc(const double2* p, double2 (&v)[VEC]) {
+template <int VEC, bool CG = false> __device__ __forceinline__ void ldc(const double2* p, double2 (&v)[VEC]) {
 #pragma unroll
-    for (int i = 0; i < VEC; ++i) v[i] = __ldg(p + i);
+    for (int i = 0; i < VEC; ++i) v[i] = ldx<CG>(p + i);
 }
 template <int VEC> __device__ __forceinline__ void stc(float2* p, const float2 (&v)[VEC]) {
     if constexpr (VEC % 2 == 0) {
@@ -75,14 +84,14 @@ template <int VEC> __device__ __forceinline__ void stc(double2* p, const double2
 #pragma unroll
     for (int i = 0; i < VEC; ++i) p[i] = v[i];
 }
-template <int VEC> __device__ __forceinline__ void ldr(const float* p, float (&v)[VEC]) {
-    if constexpr (VEC == 4) { const float4 q = __ldg(reinterpret_cast<const float4*>(p)); v[0] = q.x; v[1] = q.y; v[2] = q.z; v[3] = q.w; }
-    else if constexpr (VEC == 2) { const float2 q = __ldg(reinterpret_cast<const float2*>(p)); v[0] = q.x; v[1] = q.y; }
-    else v[0] = __ldg(p);
+template <int VEC, bool CG = false> __device__ __forceinline__ void ldr(const float* p, float (&v)[VEC]) {
+    if constexpr (VEC == 4) { const float4 q = ldx<CG>(reinterpret_cast<const float4*>(p)); v[0] = q.x; v[1] = q.y; v[2] = q.z; v[3] = q.w; }
+    else if constexpr (VEC == 2) { const float2 q = ldx<CG>(reinterpret_cast<const float2*>(p)); v[0] = q.x; v[1] = q.y; }
+    else v[0] = ldx<CG>(p);
 }
-template <int VEC> __device__ __forceinline__ void ldr(const double* p, double (&v)[VEC]) {
-    if constexpr (VEC == 2) { const double2 q = __ldg(reinterpret_cast<const double2*>(p)); v[0] = q.x; v[1] = q.y; }
-    else v[0] = __ldg(p);
+template <int VEC, bool CG = false> __device__ __forceinline__ void ldr(const double* p, double (&v)[VEC]) {
+    if constexpr (VEC == 2) { const double2 q = ldx<CG>(reinterpret_cast<const double2*>(p)); v[0] = q.x; v[1] = q.y; }
+    else v[0] = ldx<CG>(p);
 }
 template <int VEC> __device__ __forceinline__ void str(float* p, const float (&v)[VEC]) {
     if constexpr (VEC == 4) *reinterpret_cast<float4*>(p) = make_float4(v[0], v[1], v[2], v[3]);
@@ -154,6 +163,48 @@ template <int VEC> __device__ __forceinline__ void ldsr(const double* p, double 
     else v[0] = *p;
 }
 
+// Shared-memory accesses of the exchanging strips: volatile, so that the compiler keeps them in program order; the LSU
+// executes the shared-memory instructions of a warp in order, and that is all the ordering the protocol needs (a fence
+// here would also wait for the global loads in flight, which the row loop keeps in flight on purpose; measured: 67 against
+// 88 Gcell*step/s on cfg5 with __threadfence_block()).  No "memory" clobber: volatile asm statements keep their order among
+// themselves, and the global loads and stores of the row loop stay free to move across them.
+__device__ __forceinline__ void xst(float2* p, float2 v) { asm volatile("st.volatile.shared.v2.f32 [%0], {%1, %2};" ::"r"(smem_u32(p)), "f"(v.x), "f"(v.y)); }
+__device__ __forceinline__ void xst(double2* p, double2 v) { asm volatile("st.volatile.shared.v2.f64 [%0], {%1, %2};" ::"r"(smem_u32(p)), "d"(v.x), "d"(v.y)); }
+__device__ __forceinline__ float2 xld(const float2* p) { float2 v; asm volatile("ld.volatile.shared.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "r"(smem_u32(p))); return v; }
+__device__ __forceinline__ double2 xld(const double2* p) { double2 v; asm volatile("ld.volatile.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(smem_u32(p))); return v; }
+__device__ __forceinline__ void xst_flag(int* p, int v) { asm volatile("st.volatile.shared.s32 [%0], %1;" ::"r"(smem_u32(p)), "r"(v)); }
+__device__ __forceinline__ int xld_flag(const int* p) { int v; asm volatile("ld.volatile.shared.s32 %0, [%1];" : "=r"(v) : "r"(smem_u32(p))); return v; }
+
+// ---- persistent launch (template switch PERS): a warp's tile (strip, chunk, realisation) may start step s of the launch once
+// every tile whose rows or columns it reads (and whose halo reads cover the cells it is about to overwrite) has finished step
+// s-1: the 5 x 5 tiles around it, wrapped (two on either side, so that a ragged last strip or chunk of fewer than 4 cells is
+// covered).  One lane per neighbour polls its counter with ld.acquire.gpu; a counter that does not arrive within seconds traps
+// (cannot happen under a cooperative launch, where all tiles are resident; the guard turns a hang into an error).
+__device__ __forceinline__ void pers_wait(const uint32_t* flags, int strips, int chunks, int strip, int chunk, int real, int lane,
+                                          uint32_t need) {
+    if (lane < 25) {
+        int sx = (strip + lane % 5 - 2) % strips, cy = (chunk + lane / 5 - 2) % chunks;
+        if (sx < 0) sx += strips;
+        if (cy < 0) cy += chunks;
+        const uint32_t* f = flags + ((size_t)real * chunks + cy) * strips + sx;
+        uint32_t v, spins = 0;
+        for (;;) {
+            asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(f) : "memory");
+            if (v >= need) break;
+            if (++spins > (1u << 22)) __trap();
+        }
+    }
+    __syncwarp();
+}
+__device__ __forceinline__ void pers_signal(uint32_t* flags, int strips, int chunks, int strip, int chunk, int real, int lane,
+                                            uint32_t done) {
+    __syncwarp();
+    if (lane == 0) {
+        __threadfence();
+        asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(flags + ((size_t)real * chunks + chunk) * strips + strip), "r"(done) : "memory");
+    }
+}
+
 // DRAM -> L2 prefetch of the line holding p (no register is tied up; the register fetch one row ahead then hits L2).
 __device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
 
@@ -165,12 +216,19 @@ __device__ __forceinline__ double2 dn1(double2 v) { return make_double2(__shfl_d
 // Neighbourhood of cell i of the centre row (rc) of a three-row window (rs = row below, rn = row above);
 // west/east of the lane's cells by shuffle.  NINE (spinor models): the corner difference Dxy4 is formed from the
 // vertical differences n - s of the neighbouring columns, so that one pair per side crosses lanes instead of two.
-template <typename T, int VEC, bool NINE>
+// XCH (the warps of a CTA tile the whole row, see step_kernel): lane 0 takes its west neighbour and lane 31 its east
+// neighbour from `edge`, the cell the neighbouring warp published in shared memory.
+template <typename T, int VEC, bool NINE, bool XCH = false>
 __device__ __forceinline__ void gather(const typename Cx<T>::type (&rs)[VEC], const typename Cx<T>::type (&rc)[VEC],
-                                       const typename Cx<T>::type (&rn)[VEC], Nbhd<T> (&nb)[VEC]) {
+                                       const typename Cx<T>::type (&rn)[VEC], Nbhd<T> (&nb)[VEC], int lane = 0,
+                                       typename Cx<T>::type edge = typename Cx<T>::type()) {
     using C = typename Cx<T>::type;
-    const C west = up1(rc[VEC - 1]);
-    const C east = dn1(rc[0]);
+    C west = up1(rc[VEC - 1]);
+    C east = dn1(rc[0]);
+    if (XCH) {
+        if (lane == 0) west = edge;
+        if (lane == 31) east = edge;
+    }
 #pragma unroll
     for (int i = 0; i < VEC; ++i) {
         nb[i].c = rc[i];
@@ -220,42 +278,81 @@ struct StepSmem {
 // MINW: resident warps per SM the register budget is sized for.  ISO: dx == dy (scalar and reservoir models only).
 // DRIVE: coherent drive E(r) exp(-i omega t) (reading Q17), shared by both components.
 // BULK: rows are fetched by TMA bulk copies into a shared-memory ring instead of register loads (periodic boundaries only).
-template <typename T, int VEC, int MODEL, bool NOISE, bool ZBC, bool ISO, bool DRIVE, int MINW, bool BULK>
-__global__ void __launch_bounds__(32 * PHX_STEP_WARPS, MINW / PHX_STEP_WARPS)
+// XCH: the warps of a CTA (a.wpc of them, at most PHX_STEP_XWARPS) tile the WHOLE periodic row, nx = wpc * W, and exchange the
+// one column a stage needs from the neighbouring strip through shared memory instead of recomputing 4 + 4 halo columns:
+// every lane owns output columns (a 256-wide grid of cfg5 costs 4 strips of 64 columns instead of 5).  What a warp consumes in
+// the iteration with front row j (the cells of psi[j], y2[j-1], y3[j-2], y4[j-3] next to its strip) its neighbours produced in
+// iteration j-1 and left in slot (j-1) & 1 of a two-slot ring; a warp enters iteration j once both neighbours have finished
+// j-1 (a progress counter per warp, polled in shared memory), so the warps of a row drift by less than one iteration and two
+// slots suffice.  Scalar and reservoir models (the TE-TM corners would need a neighbour's row of the SAME iteration), periodic.
+// PERS: a.n_steps RK4 steps in one cooperative launch; every warp keeps its tile and waits, between steps, only for the tiles
+// around it (pers_wait above) instead of for the whole grid: no launch, ramp and tail per step.  psi_in / psi_out (n_in /
+// n_out) swap roles every step; they are read through L2 (other SMs rewrite them during the launch).  Periodic, no drive.
+template <typename T, int VEC, int MODEL, bool NOISE, bool ZBC, bool ISO, bool DRIVE, int MINW, bool BULK, bool XCH = false,
+          bool PERS = false>
+__global__ void __launch_bounds__(XCH ? 32 * PHX_STEP_XWARPS : 32 * PHX_STEP_WARPS, XCH ? 1 : MINW / PHX_STEP_WARPS)
 step_kernel(const __grid_constant__ StepArgs<T> a) {
     using namespace stepk;
     using C = typename Cx<T>::type;
     constexpr bool SPINOR = model_spinor(MODEL);
     constexpr bool RES = model_reservoir(MODEL);
     constexpr int NC = SPINOR ? 2 : 1;
-    constexpr int W = 32 * VEC, OUTW = W - 8;
+    constexpr int W = 32 * VEC, OUTW = XCH ? W : W - 8;
     constexpr int RING = PHX_STEP_RING, LEAD = PHX_STEP_LEAD;
     static_assert(!(BULK && ZBC), "the bulk-copy fetch path is built for periodic boundaries");
+    static_assert(!(XCH && (BULK || ZBC || SPINOR)), "the exchanging strips are built for periodic scalar / reservoir grids");
+    static_assert(!(PERS && (BULK || ZBC || DRIVE)), "the persistent launch is built for periodic grids without drive");
     const Geom& g = a.geo;
     const Coef<T>& k = a.k;
     const int nx = g.nx, ny = g.ny;
 
     const int lane = threadIdx.x & 31;
     const int strip = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
-    const uint64_t step = *a.step_in;
-    if (blockIdx.x == 0 && blockIdx.y == 0 && blockIdx.z == 0 && threadIdx.x == 0) *a.step_out = step + 1;
-    if (strip >= a.strips) return;   // warp-uniform
+    const uint64_t step0 = PERS ? a.step0 : *a.step_in;
+    if (blockIdx.x == 0 && blockIdx.y == 0 && blockIdx.z == 0 && threadIdx.x == 0) {
+        if (PERS) { const uint64_t after = step0 + (uint64_t)a.n_steps; *const_cast<uint64_t*>(a.step_in) = after; *a.step_out = after; }
+        else *a.step_out = step0 + 1;
+    }
+    if (!XCH && strip >= a.strips) return;   // warp-uniform
+    // exchanging strips: the ring of edge cells [2 slots][4 arrays: psi, y2, y3, y4][warp][side: 0 = first cell, 1 = last cell of
+    // the strip] and the progress counters (front row of the last iteration a warp has finished)
+    typename Cx<T>::type* xe = nullptr;
+    int* xp = nullptr;
+    constexpr int XARR = PHX_STEP_XWARPS * 2;
+    if constexpr (XCH) {
+        __shared__ typename Cx<T>::type xedge_s[2 * 4 * XARR];
+        __shared__ int xprog_s[PHX_STEP_XWARPS];
+        xe = xedge_s;
+        xp = xprog_s;
+        if (threadIdx.x < PHX_STEP_XWARPS) xprog_s[threadIdx.x] = INT_MIN;
+        __syncthreads();
+    }
 
     // ---- columns of this lane ----------------------------------------------------------------------------------
-    const int xl = strip * OUTW - 4 + lane * VEC;   // unwrapped column of the lane's first cell
+    const int xl = strip * OUTW - (XCH ? 0 : 4) + lane * VEC;   // unwrapped column of the lane's first cell
     int xg = xl;                                     // column actually addressed
     bool inx = true;                                 // false: outside a zero boundary
     if (xl < 0 || xl >= nx) {
         if (ZBC && g.bc_x) { inx = false; xg = 0; }
         else { xg = xl % nx; if (xg < 0) xg += nx; }
     }
-    const bool st_lane = lane * VEC >= 4 && lane * VEC < W - 4 && xl < nx;   // lane owns output columns
+    const bool st_lane = XCH || (lane * VEC >= 4 && lane * VEC < W - 4 && xl < nx);   // lane owns output columns
 
     // ---- rows of this chunk ------------------------------------------------------------------------------------
     const int r0 = blockIdx.y * a.ly;
     const int r1 = min(r0 + a.ly, ny);
     const size_t boff = (size_t)blockIdx.z * g.plane;
     const bool zy = ZBC && g.bc_y;
+
+    // ---- the steps of this launch (one, unless PERS) ---------------------------------------------------------------------------
+#pragma unroll 1
+    for (int it = 0; it < (PERS ? a.n_steps : 1); ++it) {
+    const uint64_t step = step0 + (uint64_t)it;
+    const bool swapped = PERS && (it & 1);      // odd steps of a persistent launch read what the even ones wrote
+    const int xkey = PERS ? it * (a.ly + 16) : 0;   // (XCH) keeps the warps' progress counters monotonic from step to step
+    if constexpr (PERS) {
+        if (it > 0) pers_wait(a.flags, a.strips, (int)gridDim.y, strip, (int)blockIdx.y, (int)blockIdx.z, lane, (uint32_t)it);
+    }
 
     // drive: q_s = (1/hbar) exp(-i omega t_s) at the stage times t, t + dt/2, t + dt, t = step dt; the phase is evaluated
     // in double and rounded to T (reading Q17)
@@ -276,10 +373,10 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
     T* nout_p[NC];
 #pragma unroll
     for (int s = 0; s < NC; ++s) {
-        pin[s] = a.psi_in[s] + boff;
-        pout[s] = a.psi_out[s] + boff;
-        nin[s] = RES ? a.n_in[s] + boff : nullptr;
-        nout_p[s] = RES ? a.n_out[s] + boff : nullptr;
+        pin[s] = (swapped ? a.psi_out[s] : a.psi_in[s]) + boff;
+        pout[s] = (swapped ? const_cast<C*>(a.psi_in[s]) : a.psi_out[s]) + boff;
+        nin[s] = RES ? (swapped ? a.n_out[s] : a.n_in[s]) + boff : nullptr;
+        nout_p[s] = RES ? (swapped ? const_cast<T*>(a.n_in[s]) : a.n_out[s]) + boff : nullptr;
     }
     const T* Vp = a.V;
     const T* Pp = RES ? a.P : nullptr;
@@ -358,7 +455,7 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
         const bool okq = !ZBC || (inx && (!zy || (qw >= 0 && qw < ny)));
 #pragma unroll
         for (int s = 0; s < NC; ++s) {
-            if (okq) ldc<VEC>(pin[s] + ew, psr[s][(d + R2) % RING]);
+            if (okq) ldc<VEC, PERS>(pin[s] + ew, psr[s][(d + R2) % RING]);
         }
         if (d >= 0 && d < LEAD && okq) {
             if (Vp) ldr<VEC>(Vp + ew, Vr[(d + R2) % RING]);
@@ -366,13 +463,31 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
             if (DRIVE) ldc<VEC>(Ep + ew, Er[(d + R2) % RING]);
             if constexpr (RES) {
 #pragma unroll
-                for (int s = 0; s < NC; ++s) ldr<VEC>(nin[s] + ew, nr[s][(d + R2) % RING]);
+                for (int s = 0; s < NC; ++s) ldr<VEC, PERS>(nin[s] + ew, nr[s][(d + R2) % RING]);
             }
         }
         ewp = ew;
         okprev = okq;
         ++qw; ew += nx;
         if (!zy && qw == ny) { qw = 0; ew -= plane; }
+    }
+
+    // ---- exchanging strips: neighbours, this lane's slots, and psi[j0] (the centre row of stage 1 in the first iteration)
+    // published as the product of "iteration j0 - 1" ---------------------------------------------------------------------------
+    int xleft = 0, xright = 0, xrd = 0, xwr = 0;
+    const bool xlane = lane == 0 || lane == 31;
+    if constexpr (XCH) {
+        const int nw = blockDim.x >> 5;
+        xleft = strip == 0 ? nw - 1 : strip - 1;
+        xright = strip == nw - 1 ? 0 : strip + 1;
+        xrd = lane == 0 ? xleft * 2 + 1 : xright * 2;   // lane 0 reads the last cell of the strip to the west, lane 31 the first of the strip to the east
+        xwr = strip * 2 + (lane == 0 ? 0 : 1);
+        if (xlane) xst(xe + (((j0 - 1) & 1) * 4 + 0) * XARR + xwr, lane == 0 ? psr[0][0][0] : psr[0][0][VEC - 1]);
+#if PHX_XCH_SYNC == 1
+        __syncthreads();
+#else
+        if (lane == 0) xst_flag(xp + strip, j0 - 1 + xkey);
+#endif
     }
 
     // ---- bulk-copy fetch path: the ring, its mbarriers and the issuer's state ------------------------------------------------
@@ -445,7 +560,18 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
     for (int jb = j0; jb <= r1 + 2; jb += RING) {
 #pragma unroll
         for (int ph = 0; ph < RING; ++ph) {
-            const int j = jb + ph;          // front row of this iteration (rows past r1+2 in the last pass are computed and not stored)
+            const int j = jb + ph;          // front row of this iteration
+            if constexpr (!BULK && !XCH && step_early_exit(sizeof(T) == 8, MODEL, VEC)) {
+                if (ph > 0 && j > r1 + 2) break;   // (warp-uniform) the chunk is done: row r1-1 was stored in the iteration with front row r1+2
+            }
+            C xin[4];                       // (XCH) the neighbours' cells next to this lane's strip: of psi[j], y2[j-1], y3[j-2], y4[j-3]
+            if constexpr (XCH) {
+#if PHX_XCH_SYNC == 0
+                while (xld_flag(xp + xleft) < j - 1 + xkey || xld_flag(xp + xright) < j - 1 + xkey) { }   // both finished iteration j-1
+#endif
+#pragma unroll
+                for (int q = 0; q < 4; ++q) xin[q] = xld(xe + (((j - 1) & 1) * 4 + q) * XARR + xrd);
+            }
             if (PF > 0 && !BULK) {
                 if (!ZBC) {
                     uint32_t e = ew + epf;                   // row qw + pfr, wrapped
@@ -495,7 +621,7 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
 #pragma unroll
                     for (int i = 0; i < VEC; ++i) psr[s][SL(1 + LEAD)][i] = czero;
                 }
-                if (okq) ldc<VEC>(pin[s] + ew, psr[s][SL(1 + LEAD)]);
+                if (okq) ldc<VEC, PERS>(pin[s] + ew, psr[s][SL(1 + LEAD)]);
             }
             if (ZBC) {              // (periodic without V or P: the slots keep the zeros they were initialised with)
 #pragma unroll
@@ -513,7 +639,7 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
 #pragma unroll
                         for (int i = 0; i < VEC; ++i) nr[s][SL(LEAD)][i] = T(0);
                     }
-                    if (okprev) ldr<VEC>(nin[s] + ewp, nr[s][SL(LEAD)]);
+                    if (okprev) ldr<VEC, PERS>(nin[s] + ewp, nr[s][SL(LEAD)]);
                 }
             }
             }
@@ -536,7 +662,7 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
 
                 // ---- stage 1: K1 on row j from psi rows j-1, j, j+1 (Eq. (2)) ---------------------------------------------
 #pragma unroll
-                for (int s = 0; s < NC; ++s) gather<T, VEC, SPINOR>(psr[s][SL(-1)], psr[s][SL(0)], psr[s][SL(1)], nb[s]);
+                for (int s = 0; s < NC; ++s) gather<T, VEC, SPINOR, XCH>(psr[s][SL(-1)], psr[s][SL(0)], psr[s][SL(1)], nb[s], lane, xin[0]);
                 diffs(nb, df);
 #pragma unroll
                 for (int s = 0; s < NC; ++s) {
@@ -544,7 +670,7 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
                     for (int i = 0; i < VEC; ++i) {
                         T Kn;
                         const T nres = RES ? nr[s][SL(0)][i] : T(0);
-                        const C K = deriv<T, SPINOR, RES, DRIVE>(k, nb[s][i].c, df[s][i], nb[O(s)][i].c, df[O(s)][i], s == 0, nres, Vr[SL(0)][i], Pr[SL(0)][i], Er[SL(0)][i], q1, Kn);
+                        const C K = deriv<T, SPINOR, RES, DRIVE, ISO>(k, nb[s][i].c, df[s][i], nb[O(s)][i].c, df[O(s)][i], s == 0, nres, Vr[SL(0)][i], Pr[SL(0)][i], Er[SL(0)][i], q1, Kn);
                         const C p = psr[s][SL(0)][i];
                         y2r[s][SL(0)][i] = in1 ? fma2s(k.hdt, K, p) : czero;
                         accr[s][SL(0)][i] = fma2s(k.dt6, K, p);
@@ -552,9 +678,16 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
                     }
                 }
 
+                if constexpr (XCH) {        // publish the edge cells of psi[j+1] and y2[j] (centre rows of stages 1, 2 in iteration j+1)
+                    if (xlane) {
+                        xst(xe + ((j & 1) * 4 + 0) * XARR + xwr, lane == 0 ? psr[0][SL(1)][0] : psr[0][SL(1)][VEC - 1]);
+                        xst(xe + ((j & 1) * 4 + 1) * XARR + xwr, lane == 0 ? y2r[0][SL(0)][0] : y2r[0][SL(0)][VEC - 1]);
+                    }
+                }
+
                 // ---- stage 2: K2 on row j-1 from y2 rows j-2, j-1, j (Eq. (3)) --------------------------------------------
 #pragma unroll
-                for (int s = 0; s < NC; ++s) gather<T, VEC, SPINOR>(y2r[s][SL(-2)], y2r[s][SL(-1)], y2r[s][SL(0)], nb[s]);
+                for (int s = 0; s < NC; ++s) gather<T, VEC, SPINOR, XCH>(y2r[s][SL(-2)], y2r[s][SL(-1)], y2r[s][SL(0)], nb[s], lane, xin[1]);
                 diffs(nb, df);
 #pragma unroll
                 for (int s = 0; s < NC; ++s) {
@@ -562,7 +695,7 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
                     for (int i = 0; i < VEC; ++i) {
                         T Kn;
                         const T nres = RES ? n2r[s][SL(-1)][i] : T(0);
-                        const C K = deriv<T, SPINOR, RES, DRIVE>(k, nb[s][i].c, df[s][i], nb[O(s)][i].c, df[O(s)][i], s == 0, nres, Vr[SL(-1)][i], Pr[SL(-1)][i], Er[SL(-1)][i], q23, Kn);
+                        const C K = deriv<T, SPINOR, RES, DRIVE, ISO>(k, nb[s][i].c, df[s][i], nb[O(s)][i].c, df[O(s)][i], s == 0, nres, Vr[SL(-1)][i], Pr[SL(-1)][i], Er[SL(-1)][i], q23, Kn);
                         const C p = psr[s][SL(-1)][i];
                         y3r[s][SL(-1)][i] = in2 ? fma2s(k.hdt, K, p) : czero;
                         accr[s][SL(-1)][i] = fma2s(k.dt3, K, accr[s][SL(-1)][i]);
@@ -570,9 +703,13 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
                     }
                 }
 
+                if constexpr (XCH) {
+                    if (xlane) xst(xe + ((j & 1) * 4 + 2) * XARR + xwr, lane == 0 ? y3r[0][SL(-1)][0] : y3r[0][SL(-1)][VEC - 1]);
+                }
+
                 // ---- stage 3: K3 on row j-2 from y3 rows j-3, j-2, j-1 (Eq. (4)) ------------------------------------------
 #pragma unroll
-                for (int s = 0; s < NC; ++s) gather<T, VEC, SPINOR>(y3r[s][SL(-3)], y3r[s][SL(-2)], y3r[s][SL(-1)], nb[s]);
+                for (int s = 0; s < NC; ++s) gather<T, VEC, SPINOR, XCH>(y3r[s][SL(-3)], y3r[s][SL(-2)], y3r[s][SL(-1)], nb[s], lane, xin[2]);
                 diffs(nb, df);
 #pragma unroll
                 for (int s = 0; s < NC; ++s) {
@@ -580,7 +717,7 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
                     for (int i = 0; i < VEC; ++i) {
                         T Kn;
                         const T nres = RES ? n3r[s][SL(-2)][i] : T(0);
-                        const C K = deriv<T, SPINOR, RES, DRIVE>(k, nb[s][i].c, df[s][i], nb[O(s)][i].c, df[O(s)][i], s == 0, nres, Vr[SL(-2)][i], Pr[SL(-2)][i], Er[SL(-2)][i], q23, Kn);
+                        const C K = deriv<T, SPINOR, RES, DRIVE, ISO>(k, nb[s][i].c, df[s][i], nb[O(s)][i].c, df[O(s)][i], s == 0, nres, Vr[SL(-2)][i], Pr[SL(-2)][i], Er[SL(-2)][i], q23, Kn);
                         const C p = psr[s][SL(-2)][i];
                         y4r[s][SL(-2)][i] = in3 ? fma2s(k.dt, K, p) : czero;
                         accr[s][SL(-2)][i] = fma2s(k.dt3, K, accr[s][SL(-2)][i]);
@@ -588,9 +725,18 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
                     }
                 }
 
+                if constexpr (XCH) {
+                    if (xlane) xst(xe + ((j & 1) * 4 + 3) * XARR + xwr, lane == 0 ? y4r[0][SL(-2)][0] : y4r[0][SL(-2)][VEC - 1]);
+#if PHX_XCH_SYNC == 1
+                    asm volatile("bar.sync 1, %0;" ::"r"((int)blockDim.x));   // iteration j's cells are out: the warps of the row step together
+#else
+                    if (lane == 0) xst_flag(xp + strip, j + xkey);                             // iteration j's cells are out
+#endif
+                }
+
                 // ---- stage 4: K4 on row j-3 from y4 rows j-4, j-3, j-2; psi(t+dt) of Eq. (6) (+ dW of Eq. (22)) ----------
 #pragma unroll
-                for (int s = 0; s < NC; ++s) gather<T, VEC, SPINOR>(y4r[s][SL(-4)], y4r[s][SL(-3)], y4r[s][SL(-2)], nb[s]);
+                for (int s = 0; s < NC; ++s) gather<T, VEC, SPINOR, XCH>(y4r[s][SL(-4)], y4r[s][SL(-3)], y4r[s][SL(-2)], nb[s], lane, xin[3]);
                 diffs(nb, df);
                 const int jr = j - 3;
                 const bool st_row = jr >= r0 && jr < r1;
@@ -603,7 +749,7 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
                     for (int i = 0; i < VEC; ++i) {
                         T Kn;
                         const T nres = RES ? n4r[s][SL(-3)][i] : T(0);
-                        const C K = deriv<T, SPINOR, RES, DRIVE>(k, nb[s][i].c, df[s][i], nb[O(s)][i].c, df[O(s)][i], s == 0, nres, Vr[SL(-3)][i], Pr[SL(-3)][i], Er[SL(-3)][i], q4, Kn);
+                        const C K = deriv<T, SPINOR, RES, DRIVE, ISO>(k, nb[s][i].c, df[s][i], nb[O(s)][i].c, df[O(s)][i], s == 0, nres, Vr[SL(-3)][i], Pr[SL(-3)][i], Er[SL(-3)][i], q4, Kn);
                         out[i] = fma2s(k.dt6, K, accr[s][SL(-3)][i]);
                         nout[i] = RES ? naccr[s][SL(-3)][i] + k.dt6 * Kn : T(0);
                     }
@@ -641,6 +787,8 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
             if (!zy && qw == ny) { qw = 0; ew -= plane; }
         }
     }
+    if constexpr (PERS) pers_signal(a.flags, a.strips, (int)gridDim.y, strip, (int)blockIdx.y, (int)blockIdx.z, lane, (uint32_t)(it + 1));
+    }   // steps of this launch
 #undef SL
 }
 

@@ -209,6 +209,106 @@ def test_spinor_noise():
     run_pair(w, 30)
 
 
+# ---- exchanging strips (the warps of a CTA tile the whole row) and the persistent launch -------------------
+def _fields(g, w):
+    return {name: g.read_field(name) for name in w.fields}
+
+
+@pytest.mark.parametrize("prec,nx,vec", [("c32", 64, 2), ("c32", 128, 2), ("c32", 256, 2), ("c32", 512, 2), ("c32", 128, 4),
+                                         ("c32", 1024, 4), ("c64", 32, 1), ("c64", 96, 1), ("c64", 256, 1), ("c64", 128, 2)])
+def test_exchanging_strips_scalar(prec, nx, vec):
+    # rows of 1, 2, 3, 4 and 8 strips; ragged chunks (ny = 45); against the oracle, and bit for bit against the independent
+    # strips (the same cell arithmetic: only where a neighbour's value comes from differs)
+    w = wl.cfg2(n=nx, ny=45, prec=prec)
+    g = make_gpu(w, variant=STEP, tuning={"step_xch": 1, "step_vec": vec, "step_ly": 11})
+    o = make_oracle(w)
+    g.step_rk4(41)
+    o.step_rk4(41)
+    compare(g, o, w)
+    ref = make_gpu(w, variant=STEP, tuning={"step_xch": 0, "step_vec": vec})
+    ref.step_rk4(41)
+    assert np.array_equal(g.read_field("psi_p"), ref.read_field("psi_p"))
+    g.destroy()
+    ref.destroy()
+
+
+@pytest.mark.parametrize("prec", ["c32", "c64"])
+def test_exchanging_strips_noisy_reservoir_ensemble(prec):
+    # cfg5's shape in small: 4 strips of 64 columns (fp64: 8 of 32), several realisations, noise, odd step count
+    w = wl.cfg5(n=256, batch=3, prec=prec)
+    g = make_gpu(w, variant=STEP, tuning={"step_xch": 1, "step_ly": 37})
+    o = make_oracle(w)
+    g.step_rk4(25)
+    o.step_rk4(25)
+    compare(g, o, w)
+    ref = make_gpu(w, variant=STEP, tuning={"step_xch": 0})
+    ref.step_rk4(25)
+    for name in w.fields:
+        assert np.array_equal(g.read_field(name), ref.read_field(name)), name
+    g.destroy()
+    ref.destroy()
+
+
+def test_exchanging_strips_are_the_default_for_ensembles_of_narrow_grids():
+    # AUTO: a million cells or more in rows of at most four strips; same bits either way
+    w = wl.cfg5(n=128, batch=64, prec="c32")
+    g = make_gpu(w, variant=STEP)
+    ref = make_gpu(w, variant=STEP, tuning={"step_xch": 0})
+    g.step_rk4(7)
+    ref.step_rk4(7)
+    for name in w.fields:
+        assert np.array_equal(g.read_field(name), ref.read_field(name)), name
+    g.destroy()
+    ref.destroy()
+
+
+@pytest.mark.parametrize("maker,tuning", [
+    (lambda: wl.cfg2(n=300, ny=70, prec="c32"), {}), (lambda: wl.cfg2(n=200, ny=64, prec="c64"), {"step_ly": 9}),
+    (lambda: wl.cfg3(n=160, prec="c32"), {"step_ly": 23}), (lambda: wl.cfg4(n=120, prec="c32", sigma_cells=10.0), {}),
+    (lambda: wl.cfg5(n=64, batch=5, prec="c32"), {}), (lambda: wl.cfg5(n=128, batch=3, prec="c32"), {"step_xch": 1}),
+    (lambda: wl.cfg2(n=2048, ny=40, prec="c32"), {"step_ly": 8})])
+def test_persistent_launch(maker, tuning):
+    # step_persist = 1: all steps of a call in ONE cooperative launch, the tiles synchronised by neighbour flags; against the
+    # oracle, bit for bit against one launch per step, odd and even step counts, and continued by ordinary steps
+    w = maker()
+    g = make_gpu(w, variant=STEP, tuning=dict(tuning, step_persist=1))
+    ref = make_gpu(w, variant=STEP, tuning=tuning)
+    o = make_oracle(w)
+    g.step_rk4(21)
+    assert g.get_launch_count() == 1
+    g.step_rk4(10)
+    assert g.get_launch_count() == 2
+    g.step_rk4(1)                                   # a single step takes the ordinary launch
+    ref.step_rk4(32)
+    o.step_rk4(32)
+    compare(g, o, w)
+    for name in w.fields:
+        assert np.array_equal(g.read_field(name), ref.read_field(name)), name
+    assert g.get_step() == 32
+    g.destroy()
+    ref.destroy()
+
+
+@pytest.mark.parametrize("maker", [lambda: wl.cfg2(n=2048, ny=40, prec="c32"), lambda: wl.cfg2(n=300, ny=70, prec="c32"),
+                                   lambda: wl.cfg2(n=200, ny=64, prec="c64"), lambda: wl.cfg3(n=160, prec="c32"),
+                                   lambda: wl.cfg4(n=120, prec="c32", sigma_cells=10.0), lambda: wl.cfg5(n=64, batch=5, prec="c32")])
+def test_bulk_copy_fetch_path(maker):
+    # step_bulk = 1: rows fetched by TMA bulk copies into a shared-memory ring (profiles/r02_tma_vs_register_fetch.md);
+    # the same cell arithmetic as the register loads: the same bits; strips that wrap around the periodic edge included
+    w = maker()
+    g = make_gpu(w, variant=STEP, tuning={"step_bulk": 1, "step_xch": 0})
+    ref = make_gpu(w, variant=STEP, tuning={"step_xch": 0})
+    o = make_oracle(w)
+    g.step_rk4(23)
+    ref.step_rk4(23)
+    o.step_rk4(23)
+    compare(g, o, w)
+    for name in w.fields:
+        assert np.array_equal(g.read_field(name), ref.read_field(name)), name
+    g.destroy()
+    ref.destroy()
+
+
 # ---- invariants (no oracle) --------------------------------------------------------------------------------
 @pytest.mark.parametrize("model", ["scalar", "reservoir", "spinor", "spinor_reservoir"])
 def test_shift_equivariance_bit_exact(model):

@@ -69,7 +69,9 @@ __device__ __forceinline__ void differences(const Coef<T>& k, const Nbhd<T>& nb,
 //   y, own:  this component's value and differences;  yo, oth: the other component's (SPINOR only)
 //   upper:   true for the psi_+ equation (operator (d_x - i d_y)^2 acts on psi_-)
 //   Ed, q:  drive amplitude E(r) of the cell and q = (1/hbar) exp(-i omega t_s) (DRIVE only):  K += -i q E
-template <typename T, bool SPINOR, bool RES, bool DRIVE, bool ISO = false>
+//   UNITH:  ih == 1 exactly (units with hbar = 1, as Eq. (1) is benchmarked: BASELINE configs 1, 2, 4): the product ih * pot is
+//           pot itself, bit for bit, and its multiplication is not issued
+template <typename T, bool SPINOR, bool RES, bool DRIVE, bool ISO = false, bool UNITH = false>
 __device__ __forceinline__ typename Cx<T>::type deriv(const Coef<T>& k, typename Cx<T>::type y, const Diff<T>& own,
                                                       typename Cx<T>::type yo, const Diff<T>& oth, bool upper, T nres, T V,
                                                       T P, typename Cx<T>::type Ed, typename Cx<T>::type q, T& Kn) {
@@ -78,7 +80,7 @@ __device__ __forceinline__ typename Cx<T>::type deriv(const Coef<T>& k, typename
     T pot = fma(k.g, rho, V);
     if (RES) pot = fma(k.gr, nres, pot);
     if (SPINOR) pot = fma(k.gx, fma(yo.y, yo.y, fma(yo.x, yo.x, -k.doff)), pot);
-    const T W = k.ih * pot;
+    const T W = UNITH ? pot : k.ih * pot;
     const T gain = RES ? fma(T(0.5) * k.Rr, nres, -k.hgc) : -k.hgc;
     // K = i M + gain y -+ bxy Dxy4[other],  M = L - W y - bxx Dxx[other] + byy Dyy[other]
     // (-i J with J = bxx Dxx - byy Dyy -+ i bxy Dxy4 of the other component; the one rotation sits on the addend

@@ -28,6 +28,10 @@
 #ifndef PHX_STEP_PF_ROWS
 #define PHX_STEP_PF_ROWS 4
 #endif
+// Second prefetch level (L2 -> L1) this many row iterations ahead of the register fetch; 0 = none.
+#ifndef PHX_STEP_PF1_ROWS
+#define PHX_STEP_PF1_ROWS 0
+#endif
 
 namespace phx {
 
@@ -207,6 +211,7 @@ __device__ __forceinline__ void pers_signal(uint32_t* flags, int strips, int chu
 
 // DRAM -> L2 prefetch of the line holding p (no register is tied up; the register fetch one row ahead then hits L2).
 __device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
+__device__ __forceinline__ void prefetch_l1(const void* p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
 
 __device__ __forceinline__ float2 up1(float2 v) { return make_float2(__shfl_up_sync(0xffffffffu, v.x, 1), __shfl_up_sync(0xffffffffu, v.y, 1)); }
 __device__ __forceinline__ float2 dn1(float2 v) { return make_float2(__shfl_down_sync(0xffffffffu, v.x, 1), __shfl_down_sync(0xffffffffu, v.y, 1)); }
@@ -288,8 +293,10 @@ struct StepSmem {
 // PERS: a.n_steps RK4 steps in one cooperative launch; every warp keeps its tile and waits, between steps, only for the tiles
 // around it (pers_wait above) instead of for the whole grid: no launch, ramp and tail per step.  psi_in / psi_out (n_in /
 // n_out) swap roles every step; they are read through L2 (other SMs rewrite them during the launch).  Periodic, no drive.
+// UNITH: hbar = 1 exactly, so that 1/hbar times the potential is the potential (phx_deriv.cuh): one FP32 instruction fewer per
+// cell and stage of the 17 the scalar model issues.
 template <typename T, int VEC, int MODEL, bool NOISE, bool ZBC, bool ISO, bool DRIVE, int MINW, bool BULK, bool XCH = false,
-          bool PERS = false>
+          bool PERS = false, bool UNITH = false>
 __global__ void __launch_bounds__(XCH ? 32 * PHX_STEP_XWARPS : 32 * PHX_STEP_WARPS, XCH ? 1 : MINW / PHX_STEP_WARPS)
 step_kernel(const __grid_constant__ StepArgs<T> a) {
     using namespace stepk;
@@ -584,6 +591,18 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
                     if (Vp) prefetch_l2(Vp + e);
                     if (Pp) prefetch_l2(Pp + e);
                     if (DRIVE) prefetch_l2(Ep + e);
+#if PHX_STEP_PF1_ROWS > 0
+                    // L2 -> L1: the row the register fetch takes PF1 iterations from now (its L2 latency is then off the fetch)
+                    uint32_t e1 = ew + (uint32_t)(PHX_STEP_PF1_ROWS * nx);
+                    if (qw + PHX_STEP_PF1_ROWS >= ny) e1 -= plane;
+#pragma unroll
+                    for (int s = 0; s < NC; ++s) {
+                        prefetch_l1(pin[s] + e1);
+                        if (RES) prefetch_l1(nin[s] + e1);
+                    }
+                    if (Vp) prefetch_l1(Vp + e1);
+                    if (Pp) prefetch_l1(Pp + e1);
+#endif
                 } else if (inx && (j + 1 + LEAD + pfr <= r1 + 3) && qw + pfr < ny && qw + pfr >= 0) {
 #pragma unroll
                     for (int s = 0; s < NC; ++s) {
@@ -670,7 +689,7 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
                     for (int i = 0; i < VEC; ++i) {
                         T Kn;
                         const T nres = RES ? nr[s][SL(0)][i] : T(0);
-                        const C K = deriv<T, SPINOR, RES, DRIVE, ISO>(k, nb[s][i].c, df[s][i], nb[O(s)][i].c, df[O(s)][i], s == 0, nres, Vr[SL(0)][i], Pr[SL(0)][i], Er[SL(0)][i], q1, Kn);
+                        const C K = deriv<T, SPINOR, RES, DRIVE, ISO, UNITH>(k, nb[s][i].c, df[s][i], nb[O(s)][i].c, df[O(s)][i], s == 0, nres, Vr[SL(0)][i], Pr[SL(0)][i], Er[SL(0)][i], q1, Kn);
                         const C p = psr[s][SL(0)][i];
                         y2r[s][SL(0)][i] = in1 ? fma2s(k.hdt, K, p) : czero;
                         accr[s][SL(0)][i] = fma2s(k.dt6, K, p);
@@ -695,7 +714,7 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
                     for (int i = 0; i < VEC; ++i) {
                         T Kn;
                         const T nres = RES ? n2r[s][SL(-1)][i] : T(0);
-                        const C K = deriv<T, SPINOR, RES, DRIVE, ISO>(k, nb[s][i].c, df[s][i], nb[O(s)][i].c, df[O(s)][i], s == 0, nres, Vr[SL(-1)][i], Pr[SL(-1)][i], Er[SL(-1)][i], q23, Kn);
+                        const C K = deriv<T, SPINOR, RES, DRIVE, ISO, UNITH>(k, nb[s][i].c, df[s][i], nb[O(s)][i].c, df[O(s)][i], s == 0, nres, Vr[SL(-1)][i], Pr[SL(-1)][i], Er[SL(-1)][i], q23, Kn);
                         const C p = psr[s][SL(-1)][i];
                         y3r[s][SL(-1)][i] = in2 ? fma2s(k.hdt, K, p) : czero;
                         accr[s][SL(-1)][i] = fma2s(k.dt3, K, accr[s][SL(-1)][i]);
@@ -717,7 +736,7 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
                     for (int i = 0; i < VEC; ++i) {
                         T Kn;
                         const T nres = RES ? n3r[s][SL(-2)][i] : T(0);
-                        const C K = deriv<T, SPINOR, RES, DRIVE, ISO>(k, nb[s][i].c, df[s][i], nb[O(s)][i].c, df[O(s)][i], s == 0, nres, Vr[SL(-2)][i], Pr[SL(-2)][i], Er[SL(-2)][i], q23, Kn);
+                        const C K = deriv<T, SPINOR, RES, DRIVE, ISO, UNITH>(k, nb[s][i].c, df[s][i], nb[O(s)][i].c, df[O(s)][i], s == 0, nres, Vr[SL(-2)][i], Pr[SL(-2)][i], Er[SL(-2)][i], q23, Kn);
                         const C p = psr[s][SL(-2)][i];
                         y4r[s][SL(-2)][i] = in3 ? fma2s(k.dt, K, p) : czero;
                         accr[s][SL(-2)][i] = fma2s(k.dt3, K, accr[s][SL(-2)][i]);
@@ -749,7 +768,7 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
                     for (int i = 0; i < VEC; ++i) {
                         T Kn;
                         const T nres = RES ? n4r[s][SL(-3)][i] : T(0);
-                        const C K = deriv<T, SPINOR, RES, DRIVE, ISO>(k, nb[s][i].c, df[s][i], nb[O(s)][i].c, df[O(s)][i], s == 0, nres, Vr[SL(-3)][i], Pr[SL(-3)][i], Er[SL(-3)][i], q4, Kn);
+                        const C K = deriv<T, SPINOR, RES, DRIVE, ISO, UNITH>(k, nb[s][i].c, df[s][i], nb[O(s)][i].c, df[O(s)][i], s == 0, nres, Vr[SL(-3)][i], Pr[SL(-3)][i], Er[SL(-3)][i], q4, Kn);
                         out[i] = fma2s(k.dt6, K, accr[s][SL(-3)][i]);
                         nout[i] = RES ? naccr[s][SL(-3)][i] + k.dt6 * Kn : T(0);
                     }

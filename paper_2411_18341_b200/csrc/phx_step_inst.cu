@@ -46,14 +46,14 @@ typedef double real_t;
 #define PHX_HAS_VEC4 (PHX_INST_PREC == 32 && PHX_INST_MODEL == 0)
 #endif
 
-template <int VEC, bool NOISE, bool ZBC, bool ISO, bool DRIVE, bool BULK>
+template <int VEC, bool NOISE, bool ZBC, bool ISO, bool DRIVE, bool BULK, bool UNITH = false>
 struct Inst {
     // (the noisy reservoir kernel, cfg5, is 9 % faster with the registers of 8 resident warps than with those of 12)
     static constexpr int MINW = VEC == 4 ? PHX_MINW_V4 : (VEC == 2 ? ((NOISE && PHX_INST_MODEL == 1 && PHX_INST_PREC == 32) ? 8 : PHX_MINW_V2) : PHX_MINW_V1);
     static constexpr bool I = ISO && PHX_HAS_ISO;
     // dynamic shared memory: the per-warp rings of the bulk-copy fetch path
     static constexpr size_t SMEM = BULK ? StepSmem<real_t, VEC, PHX_INST_MODEL, DRIVE>::CTA : 0;
-    static auto kernel() { return step_kernel<real_t, VEC, PHX_INST_MODEL, NOISE, ZBC, I, DRIVE, MINW, BULK, false, PHX_INST_PERS != 0>; }
+    static auto kernel() { return step_kernel<real_t, VEC, PHX_INST_MODEL, NOISE, ZBC, I, DRIVE, MINW, BULK, false, PHX_INST_PERS != 0, UNITH>; }
     static cudaError_t prepare() {
         if (SMEM > 48 * 1024) {
             static cudaError_t once = cudaFuncSetAttribute(kernel(), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM);
@@ -85,36 +85,41 @@ struct Inst {
 };
 
 // (the bulk-copy fetch path exists for periodic boundaries; a grid with a zero boundary takes the register loads)
+// unith: hbar == 1 exactly; instantiated for the isotropic periodic kernels without drive (the BASELINE grids), the others
+// multiply by 1.0f -- the same bits.
 template <int VEC, bool NOISE, bool DRIVE, typename F>
-static auto dispatch2(bool zbc, bool iso, bool bulk, F f) {
+static auto dispatch2(bool zbc, bool iso, bool bulk, bool unith, F f) {
 #if PHX_INST_PERS
     return iso ? f(Inst<VEC, NOISE, false, true, false, false>()) : f(Inst<VEC, NOISE, false, false, false, false>());
 #else
     if (zbc) return iso ? f(Inst<VEC, NOISE, true, true, DRIVE, false>()) : f(Inst<VEC, NOISE, true, false, DRIVE, false>());
     if (bulk) return iso ? f(Inst<VEC, NOISE, false, true, DRIVE, true>()) : f(Inst<VEC, NOISE, false, false, DRIVE, true>());
+    if constexpr (!DRIVE) {
+        if (unith && iso) return f(Inst<VEC, NOISE, false, true, false, false, true>());
+    }
     return iso ? f(Inst<VEC, NOISE, false, true, DRIVE, false>()) : f(Inst<VEC, NOISE, false, false, DRIVE, false>());
 #endif
 }
 
 template <int VEC, typename F>
-static auto dispatch(bool noise, bool zbc, bool iso, bool drive, bool bulk, F f) {
+static auto dispatch(bool noise, bool zbc, bool iso, bool drive, bool bulk, bool unith, F f) {
 #if PHX_INST_PERS
-    return noise ? dispatch2<VEC, true, false>(false, iso, false, f) : dispatch2<VEC, false, false>(false, iso, false, f);
+    return noise ? dispatch2<VEC, true, false>(false, iso, false, false, f) : dispatch2<VEC, false, false>(false, iso, false, false, f);
 #endif
-    if (noise && drive) return dispatch2<VEC, true, true>(zbc, iso, bulk, f);   // Eq. (16) carries E and dW together
-    if (noise) return dispatch2<VEC, true, false>(zbc, iso, bulk, f);
-    if (drive) return dispatch2<VEC, false, true>(zbc, iso, bulk, f);
-    return dispatch2<VEC, false, false>(zbc, iso, bulk, f);
+    if (noise && drive) return dispatch2<VEC, true, true>(zbc, iso, bulk, unith, f);   // Eq. (16) carries E and dW together
+    if (noise) return dispatch2<VEC, true, false>(zbc, iso, bulk, unith, f);
+    if (drive) return dispatch2<VEC, false, true>(zbc, iso, bulk, unith, f);
+    return dispatch2<VEC, false, false>(zbc, iso, bulk, unith, f);
 }
 
 template <int VEC>
 static int occ_vec(bool noise, bool zbc, bool iso, bool drive, bool bulk) {
-    return dispatch<VEC>(noise, zbc, iso, drive, bulk, [](auto inst) { return decltype(inst)::occupancy(); });
+    return dispatch<VEC>(noise, zbc, iso, drive, bulk, false, [](auto inst) { return decltype(inst)::occupancy(); });
 }
 
 template <int VEC>
 static cudaError_t launch_vec(const StepArgs<real_t>& a, bool noise, bool zbc, bool iso, bool bulk, dim3 grid, cudaStream_t st) {
-    return dispatch<VEC>(noise, zbc, iso, a.E != nullptr, bulk, [&](auto inst) { return decltype(inst)::launch(a, grid, st); });
+    return dispatch<VEC>(noise, zbc, iso, a.E != nullptr, bulk, a.k.ih == real_t(1), [&](auto inst) { return decltype(inst)::launch(a, grid, st); });
 }
 
 #define PHX_CAT3(a, b, c) a##b##_##c

@@ -91,6 +91,9 @@ struct phx_grid {
     char* ws;
     cudaStream_t stream;
     cudaStream_t cap_stream;
+    cudaStream_t side_stream;   // second branch of the captured step (the side launch of a ragged last strip)
+    cudaEvent_t ev_fork, ev_join;
+    int step_side;          // variant STEP side launch for a ragged last strip: 1 on; -1 and 0: off
     bool has_params;
     phx_params prm;
     double coef[PHX_NCOEF];
@@ -299,7 +302,24 @@ int step_occupancy(const phx_grid* g, int vec) {
     }
 }
 
-int step_strips(const phx_grid* g, int vec) { return (g->d.nx + 32 * vec - 9) / (32 * vec - 8); }
+// Ragged last strip.  The strips of 4 cells per lane produce 120 columns each: 4096 = 34 x 120 + 16, and a 35th strip (and
+// with it 33 instead of 34 chunks of rows, to stay within one wave) would be computed for 16 columns.  When the remainder is at
+// most a quarter of a strip, the main launch covers the whole strips only and a SIDE launch of the same kernel with one cell
+// per lane (strips of 32 columns, a quarter of the work per row, 80 registers: its warps fit the register space the main launch
+// leaves free) covers the remaining columns on a forked branch of the captured graph.  Only when asked for (tuning key
+// step_side = 1): measured SLOWER, 179 against 204 Gcell*step/s at 4096^2 in the same run -- the two kernels of a step do not
+// overlap (the side launch's 34 CTAs start when the main launch drains and then run alone for 11 us).
+int stepx_vec(const phx_grid* g);
+int step_side_cols(const phx_grid* g, int vec) {
+    if (g->step_side != 1 || g->step_persist == 1 || vec != 4 || stepx_vec(g) || step_bulk(g)) return 0;
+    const int outw = 32 * vec - 8, rem = g->d.nx % outw;
+    return (g->d.nx > outw && rem > 0 && rem <= outw / 4) ? rem : 0;
+}
+
+int step_strips(const phx_grid* g, int vec) {
+    const int outw = 32 * vec - 8;
+    return step_side_cols(g, vec) ? g->d.nx / outw : (g->d.nx + outw - 1) / outw;
+}
 
 // Warps per CTA: the warps of a CTA own adjacent strips and are otherwise independent.  Two per CTA measured 4 % faster
 // than one on the 16384^2 spinor and equal on the 4096^2 reservoir grid; but a row with an odd number of strips leaves the
@@ -327,7 +347,11 @@ size_t step_bytes_per_cell(const phx_grid* g) {
 //    Gcell*step/s).
 //  One warp per CTA is taken when it is at least 2 % cheaper than two by this count (4096^2 scalar fp32: 35 strips x 33
 //  chunks of 125 rows fill 1155 of 1184 warp slots, 131 iterations; in pairs 18 x 32 CTAs of 128 rows, 134 iterations).
-struct StepPlan { int ly, wpc, vec; bool xch; };
+struct StepPlan {
+    int ly, wpc, vec;
+    bool xch;
+    int side_cols;      // > 0: the last side_cols columns of every row are left to a SIDE launch of one cell per lane
+};
 
 // Exchanging strips (phx_step.cuh, XCH): cells per lane with which the warps of one CTA tile the whole row, or 0.
 // Periodic scalar / reservoir grids without drive whose width is 1 .. PHX_STEP_XWARPS strips of 32 * vec columns.
@@ -366,6 +390,7 @@ double step_plan_cost(const phx_grid* g, int vec, int wpc, int* ly_out, bool xch
                            : (long)g->n_sm * step_occupancy(g, vec) * (PHX_STEP_WARPS / wpc);   // resident CTAs of wpc warps
     const bool in_l2 = plane_cells(g) * g->d.batch * step_bytes_per_cell(g) < g->l2_bytes / 2;
     const bool whole_passes = xch || step_bulk(g) || !step_early_exit(g->d.prec == PHX_C64, g->d.model, vec);
+    const int ring = xch ? 4 + PHX_STEP_XLEAD : PHX_STEP_RING;
     double best_cost = -1;
     int best_ly = g->d.ny;
     const int max_chunks = g->d.ny / 4 > 0 ? g->d.ny / 4 : 1;   // (a 64^2 grid: ly = 4, 3.6 instead of 4.9 us per step)
@@ -375,7 +400,7 @@ double step_plan_cost(const phx_grid* g, int vec, int wpc, int* ly_out, bool xch
         const int real_chunks = (g->d.ny + ly - 1) / ly;
         const long ctas = ctas_row * real_chunks;
         const long waves = (ctas + slots - 1) / slots;
-        const long iters = whole_passes ? (ly + 6 + PHX_STEP_RING - 1) / PHX_STEP_RING * PHX_STEP_RING : ly + 6;
+        const long iters = whole_passes ? (ly + 6 + ring - 1) / ring * ring : ly + 6;
         double cost = (double)(waves * iters);
         if (in_l2) {
             const long per_sm = ((ctas + waves - 1) / waves + g->n_sm - 1) / g->n_sm;     // CTAs on the fullest SM
@@ -385,6 +410,19 @@ double step_plan_cost(const phx_grid* g, int vec, int wpc, int* ly_out, bool xch
         if (best_cost < 0 || cost < best_cost) { best_cost = cost; best_ly = ly; }
         if (g->step_ly) break;
     }
+    // Chunks that start on a multiple of 64 rows when that costs at most 2.5 % more by the count above (4096^2 fp32, same
+    // run: ly = 128 216.2, ly = 125 213.1 Gcell*step/s although 125 rows are 131 iterations against 134: the rows of a chunk
+    // boundary then start on the same DRAM page stride for every warp).
+    if (!g->step_ly && !in_l2 && best_ly % 64 != 0) {
+        const int ly = (best_ly + 63) / 64 * 64;
+        if (ly < g->d.ny) {
+            const long ctas = ctas_row * ((g->d.ny + ly - 1) / ly);
+            const long waves = (ctas + slots - 1) / slots;
+            const long iters = whole_passes ? (ly + 6 + ring - 1) / ring * ring : ly + 6;
+            const double cost = (double)(waves * iters);
+            if (cost <= best_cost * 1.025) { best_cost = cost; best_ly = ly; }
+        }
+    }
     *ly_out = best_ly;
     return best_cost;
 }
@@ -392,6 +430,7 @@ double step_plan_cost(const phx_grid* g, int vec, int wpc, int* ly_out, bool xch
 StepPlan step_plan(const phx_grid* g) {
     StepPlan p;
     p.xch = false;
+    p.side_cols = 0;
     if (const int xv = stepx_vec(g)) {
         p.xch = true;
         p.vec = xv;
@@ -400,6 +439,7 @@ StepPlan step_plan(const phx_grid* g) {
         return p;
     }
     const int vec = p.vec = step_vec(g);
+    p.side_cols = step_side_cols(g, vec);
     if (g->step_warps) {
         p.wpc = g->step_warps;
         step_plan_cost(g, vec, p.wpc, &p.ly);
@@ -488,21 +528,37 @@ cudaError_t enqueue_step_fused(phx_grid* g, cudaStream_t st, int parity, int n_p
         else
             return g->d.model == 0 ? launch_stepx_64_0(a, noise, iso, vec, grid, st) : launch_stepx_64_1(a, noise, iso, vec, grid, st);
     }
-    if constexpr (sizeof(T) == 4) {
-        switch (g->d.model) {
-            case 0: return launch_step_32_0(a, noise, zbc, iso, bulk, vec, grid, st);
-            case 1: return launch_step_32_1(a, noise, zbc, iso, bulk, vec, grid, st);
-            case 2: return launch_step_32_2(a, noise, zbc, iso, bulk, vec, grid, st);
-            default: return launch_step_32_3(a, noise, zbc, iso, bulk, vec, grid, st);
+    auto launch = [&](const StepArgs<T>& args, int v, dim3 gr, cudaStream_t stream) -> cudaError_t {
+        if constexpr (sizeof(T) == 4) {
+            switch (g->d.model) {
+                case 0: return launch_step_32_0(args, noise, zbc, iso, bulk, v, gr, stream);
+                case 1: return launch_step_32_1(args, noise, zbc, iso, bulk, v, gr, stream);
+                case 2: return launch_step_32_2(args, noise, zbc, iso, bulk, v, gr, stream);
+                default: return launch_step_32_3(args, noise, zbc, iso, bulk, v, gr, stream);
+            }
+        } else {
+            switch (g->d.model) {
+                case 0: return launch_step_64_0(args, noise, zbc, iso, bulk, v, gr, stream);
+                case 1: return launch_step_64_1(args, noise, zbc, iso, bulk, v, gr, stream);
+                case 2: return launch_step_64_2(args, noise, zbc, iso, bulk, v, gr, stream);
+                default: return launch_step_64_3(args, noise, zbc, iso, bulk, v, gr, stream);
+            }
         }
-    } else {
-        switch (g->d.model) {
-            case 0: return launch_step_64_0(a, noise, zbc, iso, bulk, vec, grid, st);
-            case 1: return launch_step_64_1(a, noise, zbc, iso, bulk, vec, grid, st);
-            case 2: return launch_step_64_2(a, noise, zbc, iso, bulk, vec, grid, st);
-            default: return launch_step_64_3(a, noise, zbc, iso, bulk, vec, grid, st);
-        }
-    }
+    };
+    if (plan.side_cols == 0) return launch(a, vec, grid, st);
+    // main launch (whole strips) and side launch (the remaining columns, one cell per lane) on two branches
+    cudaError_t e = cudaEventRecord(g->ev_fork, st);
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(g->side_stream, g->ev_fork, 0);
+    if (e == cudaSuccess) e = launch(a, vec, grid, st);
+    if (e != cudaSuccess) return e;
+    StepArgs<T> b = a;
+    b.x0 = a.strips * (32 * vec - 8);
+    b.strips = (plan.side_cols + 23) / 24;
+    b.wpc = 1;
+    e = launch(b, 1, dim3(b.strips, grid.y, grid.z), g->side_stream);
+    if (e == cudaSuccess) e = cudaEventRecord(g->ev_join, g->side_stream);
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(st, g->ev_join, 0);
+    return e;
 }
 
 // The persistent launch of the fused step: periodic grids without drive, and only when asked for (step_persist = 1).  Measured
@@ -516,7 +572,10 @@ bool persist_wanted(const phx_grid* g) {
     return !(g->d.bc_x || g->d.bc_y || g->hasE || step_bulk(g));
 }
 
-int kernels_per_step(const phx_grid* g) { return g->variant == PHX_VARIANT_STEP ? 1 : 4; }   // (RESIDENT: one per call)
+int kernels_per_step(const phx_grid* g) {
+    if (g->variant != PHX_VARIANT_STEP) return 4;
+    return step_plan(g).side_cols > 0 ? 2 : 1;      // (a ragged last strip: main + side launch)
+}   // (RESIDENT: one per call)
 
 // Variant RESIDENT: all n steps in one launch, in place on the buffers of the current parity.
 template <typename T>
@@ -760,6 +819,9 @@ phx_status phx_create_grid(phx_grid** out, const phx_grid_desc* desc) {
     g->ws = (char*)desc->workspace;
     g->stream = (cudaStream_t)desc->stream;
     g->cap_stream = nullptr;
+    g->side_stream = nullptr;
+    g->ev_fork = nullptr;
+    g->ev_join = nullptr;
     g->has_params = false;
     std::memset(&g->prm, 0, sizeof(g->prm));
     std::memset(g->coef, 0, sizeof(g->coef));
@@ -777,6 +839,7 @@ phx_status phx_create_grid(phx_grid** out, const phx_grid_desc* desc) {
     g->step_ly = g->step_vec = 0;
     g->step_bulk = -1;
     g->step_xch = -1;
+    g->step_side = -1;
     g->step_persist = -1;
     g->persist_failed = false;
     g->step_warps = 0;
@@ -787,6 +850,9 @@ phx_status phx_create_grid(phx_grid** out, const phx_grid_desc* desc) {
     g->variant = PHX_VARIANT_STAGE;
     resolve_variant(g);
     if (cudaStreamCreateWithFlags(&g->cap_stream, cudaStreamNonBlocking) != cudaSuccess) { delete g; return PHX_ERR_CUDA; }
+    if (cudaStreamCreateWithFlags(&g->side_stream, cudaStreamNonBlocking) != cudaSuccess ||
+        cudaEventCreateWithFlags(&g->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
+        cudaEventCreateWithFlags(&g->ev_join, cudaEventDisableTiming) != cudaSuccess) { delete g; return PHX_ERR_CUDA; }
     // zero the state, the static fields and the step counter
     if (cudaMemsetAsync(g->ws, 0, L.total, g->stream) != cudaSuccess) { cudaStreamDestroy(g->cap_stream); delete g; return PHX_ERR_CUDA; }
     if (desc->integrator == PHX_INT_DP54) {
@@ -1136,6 +1202,9 @@ phx_status phx_set_tuning(phx_grid* g, const char* key, int32_t value) {
     } else if (!std::strcmp(key, "step_xch")) {       // variant STEP exchanging strips: -1 automatic (wherever the row fits), 0 off
         if (value < -1 || value > 1) return PHX_ERR_INVALID_ARG;
         g->step_xch = value;
+    } else if (!std::strcmp(key, "step_side")) {      // variant STEP side launch for a ragged last strip: 1 on; -1 (automatic) and 0: off
+        if (value < -1 || value > 1) return PHX_ERR_INVALID_ARG;
+        g->step_side = value;
     } else if (!std::strcmp(key, "step_persist")) {   // variant STEP persistent launch: 1 on; -1 (automatic) and 0: off
         if (value < -1 || value > 1) return PHX_ERR_INVALID_ARG;
         g->step_persist = value;
@@ -1166,6 +1235,9 @@ void phx_destroy_grid(phx_grid* g) {
     if (!g) return;
     drop_graphs(g);
     if (g->cap_stream) cudaStreamDestroy(g->cap_stream);
+    if (g->side_stream) cudaStreamDestroy(g->side_stream);
+    if (g->ev_fork) cudaEventDestroy(g->ev_fork);
+    if (g->ev_join) cudaEventDestroy(g->ev_join);
     delete g;
 }
 

@@ -27,6 +27,11 @@
 #define PHX_STEP_LEAD 1
 #endif
 #define PHX_STEP_RING (4 + PHX_STEP_LEAD)
+// The exchanging strips fetch two rows ahead: a warp that waits for a load holds the whole row's barrier up, and the kernels
+// have the registers (cfg5: 105.0 against 102.2 Gcell*step/s).
+#ifndef PHX_STEP_XLEAD
+#define PHX_STEP_XLEAD 2
+#endif
 // Leave the unrolled row loop in the middle of its last pass (a chunk of ly rows costs ly + 6 iterations instead of the next
 // multiple of the ring length).  The exit test splits the loop body into one basic block per phase, which costs the other
 // kernels more than the saved iterations give back (same-run A/B: 4096^2 scalar fp32 4 cells per lane 213 against 205

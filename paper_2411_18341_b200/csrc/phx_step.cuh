@@ -53,6 +53,7 @@ struct StepArgs {
     int ly;                     // rows per chunk
     int strips;                 // strips per row of the grid
     int wpc;                    // warps per CTA of this launch (1 .. PHX_STEP_WARPS; the warps of a CTA are independent)
+    int x0;                     // first output column of strip 0 (0, except in the side launch that covers a ragged last strip)
     // persistent launch (template switch PERS): n_steps RK4 steps in ONE cooperative launch
     int n_steps;
     uint64_t step0;             // completed steps before this launch (the host's count; the device slots are written at the end)
@@ -230,7 +231,9 @@ __device__ __forceinline__ void gather(const typename Cx<T>::type (&rs)[VEC], co
     using C = typename Cx<T>::type;
     C west = up1(rc[VEC - 1]);
     C east = dn1(rc[0]);
-    if (XCH) {
+    if (XCH) {          // edge: read from shared memory at the top of the iteration (one load per lane: lane 0 the last cell of the
+        // strip to the west, lane 31 the first of the strip to the east) and selected in here.  Loading it here, next to its use,
+        // measured 94 against 105 Gcell*step/s on cfg5; a predicated load straight into the shuffled register (no select) 97.
         if (lane == 0) west = edge;
         if (lane == 31) east = edge;
     }
@@ -305,7 +308,7 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
     constexpr bool RES = model_reservoir(MODEL);
     constexpr int NC = SPINOR ? 2 : 1;
     constexpr int W = 32 * VEC, OUTW = XCH ? W : W - 8;
-    constexpr int RING = PHX_STEP_RING, LEAD = PHX_STEP_LEAD;
+    constexpr int LEAD = XCH ? PHX_STEP_XLEAD : PHX_STEP_LEAD, RING = 4 + LEAD;
     static_assert(!(BULK && ZBC), "the bulk-copy fetch path is built for periodic boundaries");
     static_assert(!(XCH && (BULK || ZBC || SPINOR)), "the exchanging strips are built for periodic scalar / reservoir grids");
     static_assert(!(PERS && (BULK || ZBC || DRIVE)), "the persistent launch is built for periodic grids without drive");
@@ -316,7 +319,7 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
     const int lane = threadIdx.x & 31;
     const int strip = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
     const uint64_t step0 = PERS ? a.step0 : *a.step_in;
-    if (blockIdx.x == 0 && blockIdx.y == 0 && blockIdx.z == 0 && threadIdx.x == 0) {
+    if (blockIdx.x == 0 && blockIdx.y == 0 && blockIdx.z == 0 && threadIdx.x == 0 && a.x0 == 0) {
         if (PERS) { const uint64_t after = step0 + (uint64_t)a.n_steps; *const_cast<uint64_t*>(a.step_in) = after; *a.step_out = after; }
         else *a.step_out = step0 + 1;
     }
@@ -336,7 +339,7 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
     }
 
     // ---- columns of this lane ----------------------------------------------------------------------------------
-    const int xl = strip * OUTW - (XCH ? 0 : 4) + lane * VEC;   // unwrapped column of the lane's first cell
+    const int xl = a.x0 + strip * OUTW - (XCH ? 0 : 4) + lane * VEC;   // unwrapped column of the lane's first cell
     int xg = xl;                                     // column actually addressed
     bool inx = true;                                 // false: outside a zero boundary
     if (xl < 0 || xl >= nx) {

@@ -29,13 +29,9 @@ def _units():
                       [f"-DPHX_INST_PREC={prec}", f"-DPHX_INST_MODEL={model}"]))
             u.append((f"phx_step_{prec}_{model}.o", "phx_step_inst.cu",
                       [f"-DPHX_INST_PREC={prec}", f"-DPHX_INST_MODEL={model}"]))
-            u.append((f"phx_stepp_{prec}_{model}.o", "phx_step_inst.cu",
-                      [f"-DPHX_INST_PREC={prec}", f"-DPHX_INST_MODEL={model}", "-DPHX_INST_PERS=1"]))
             if model < 2:
                 u.append((f"phx_stepx_{prec}_{model}.o", "phx_stepx_inst.cu",
                           [f"-DPHX_INST_PREC={prec}", f"-DPHX_INST_MODEL={model}"]))
-                u.append((f"phx_stepxp_{prec}_{model}.o", "phx_stepx_inst.cu",
-                          [f"-DPHX_INST_PREC={prec}", f"-DPHX_INST_MODEL={model}", "-DPHX_INST_PERS=1"]))
     return u
 
 

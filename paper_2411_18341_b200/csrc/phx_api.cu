@@ -20,11 +20,10 @@ using namespace phx;
 namespace {
 
 constexpr size_t ALIGN = 256;
-constexpr size_t FLAG_BYTES = 64 * 1024;   // progress counters of the persistent fused step: one uint32 per tile (warp)
 inline size_t align_up(size_t v) { return (v + ALIGN - 1) / ALIGN * ALIGN; }
 
 struct Layout {
-    size_t psi[2], ya[2], yb[2], acc[2], n[2], na[2], nb[2], nacc[2], V, P, E, step, flags, total;
+    size_t psi[2], ya[2], yb[2], acc[2], n[2], na[2], nb[2], nacc[2], V, P, E, step, total;
     size_t K[7][2], Kn[7][2], dpctl, dplog;   // adaptive integrator (PHX_INT_DP54 only)
     size_t scratch_bytes;   // yb[0], acc[0] are contiguous and dead between steps in every variant: scratch
 };
@@ -69,7 +68,6 @@ Layout make_layout(const phx_grid_desc* d) {
     L.P = take(plane * rb);
     L.E = take(plane * cb);
     L.step = take(ALIGN);
-    L.flags = take(FLAG_BYTES);
     if (d->integrator == PHX_INT_DP54) {
         for (int q = 0; q < 7; ++q)
             for (int s = 0; s < nc; ++s) {
@@ -108,8 +106,6 @@ struct phx_grid {
     int step_warps;         // variant STEP warps per CTA (0 = automatic)
     int step_bulk;          // variant STEP fetch path: -1 automatic, 0 register loads, 1 bulk copies into a shared-memory ring
     int step_xch;           // variant STEP exchanging strips (the warps of a CTA tile the whole row): -1 automatic, 0 off
-    int step_persist;       // variant STEP persistent launch (all steps of a call in one cooperative launch): -1 automatic, 0 off, 1 on
-    bool persist_failed;    // the cooperative launch was refused for the current plan (tiles not all resident): graphs instead
     int async_host;         // 1: host copies of set_field / read_field do not synchronise (pinned buffers, caller syncs)
     cudaGraphExec_t g1[2], gN;  // one step from parity 0 / 1; graph_steps steps from parity 0
     cudaGraphExec_t gdp;        // adaptive integrator: setup -> WHILE { seven stages, control } -> finalize
@@ -179,7 +175,6 @@ void drop_graphs(phx_grid* g) {
     if (g->gdp) cudaGraphExecDestroy(g->gdp);
     g->gdp = nullptr;
     g->graphs_valid = false;
-    g->persist_failed = false;      // (the launch plan may have changed)
 }
 
 template <typename T>
@@ -311,7 +306,7 @@ int step_occupancy(const phx_grid* g, int vec) {
 // overlap (the side launch's 34 CTAs start when the main launch drains and then run alone for 11 us).
 int stepx_vec(const phx_grid* g);
 int step_side_cols(const phx_grid* g, int vec) {
-    if (g->step_side != 1 || g->step_persist == 1 || vec != 4 || stepx_vec(g) || step_bulk(g)) return 0;
+    if (g->step_side != 1 || vec != 4 || stepx_vec(g) || step_bulk(g)) return 0;
     const int outw = 32 * vec - 8, rem = g->d.nx % outw;
     return (g->d.nx > outw && rem > 0 && rem <= outw / 4) ? rem : 0;
 }
@@ -455,10 +450,8 @@ StepPlan step_plan(const phx_grid* g) {
 }
 
 // One RK4 step of variant STEP: a single kernel that reads the state of parity p and writes parity 1-p.
-// n_persist > 0: the PERSISTENT launch instead -- n_persist steps in one cooperative launch (phx_step.cuh, PERS), the state
-// ends in parity p ^ (n_persist & 1); cudaErrorCooperativeLaunchTooLarge when the tiles are not all resident.
 template <typename T>
-cudaError_t enqueue_step_fused(phx_grid* g, cudaStream_t st, int parity, int n_persist = 0) {
+cudaError_t enqueue_step_fused(phx_grid* g, cudaStream_t st, int parity) {
     using C = typename Cx<T>::type;
     StepArgs<T> a;
     std::memset(&a, 0, sizeof(a));
@@ -492,36 +485,6 @@ cudaError_t enqueue_step_fused(phx_grid* g, cudaStream_t st, int parity, int n_p
     const dim3 grid((a.strips + a.wpc - 1) / a.wpc, (g->d.ny + a.ly - 1) / a.ly, g->d.batch);
     if (grid.y > 65535u) return cudaErrorInvalidConfiguration;
     const bool noise = g->d.noise != 0, zbc = g->d.bc_x || g->d.bc_y, iso = step_iso(g), bulk = step_bulk(g);
-    if (n_persist > 0) {
-        const size_t tiles = (size_t)a.strips * grid.y * grid.z;
-        if (zbc || bulk || g->hasE || tiles * sizeof(uint32_t) > FLAG_BYTES) return cudaErrorCooperativeLaunchTooLarge;
-        a.n_steps = n_persist;
-        a.step0 = g->step_host;
-        a.flags = (uint32_t*)(g->ws + g->L.flags);
-        cudaError_t e = cudaMemsetAsync(a.flags, 0, tiles * sizeof(uint32_t), st);
-        if (e != cudaSuccess) return e;
-        if (plan.xch) {
-            if constexpr (sizeof(T) == 4)
-                return g->d.model == 0 ? launch_stepxp_32_0(a, noise, iso, vec, grid, st) : launch_stepxp_32_1(a, noise, iso, vec, grid, st);
-            else
-                return g->d.model == 0 ? launch_stepxp_64_0(a, noise, iso, vec, grid, st) : launch_stepxp_64_1(a, noise, iso, vec, grid, st);
-        }
-        if constexpr (sizeof(T) == 4) {
-            switch (g->d.model) {
-                case 0: return launch_stepp_32_0(a, noise, zbc, iso, bulk, vec, grid, st);
-                case 1: return launch_stepp_32_1(a, noise, zbc, iso, bulk, vec, grid, st);
-                case 2: return launch_stepp_32_2(a, noise, zbc, iso, bulk, vec, grid, st);
-                default: return launch_stepp_32_3(a, noise, zbc, iso, bulk, vec, grid, st);
-            }
-        } else {
-            switch (g->d.model) {
-                case 0: return launch_stepp_64_0(a, noise, zbc, iso, bulk, vec, grid, st);
-                case 1: return launch_stepp_64_1(a, noise, zbc, iso, bulk, vec, grid, st);
-                case 2: return launch_stepp_64_2(a, noise, zbc, iso, bulk, vec, grid, st);
-                default: return launch_stepp_64_3(a, noise, zbc, iso, bulk, vec, grid, st);
-            }
-        }
-    }
     if (plan.xch) {
         if constexpr (sizeof(T) == 4)
             return g->d.model == 0 ? launch_stepx_32_0(a, noise, iso, vec, grid, st) : launch_stepx_32_1(a, noise, iso, vec, grid, st);
@@ -559,17 +522,6 @@ cudaError_t enqueue_step_fused(phx_grid* g, cudaStream_t st, int parity, int n_p
     if (e == cudaSuccess) e = cudaEventRecord(g->ev_join, g->side_stream);
     if (e == cudaSuccess) e = cudaStreamWaitEvent(st, g->ev_join, 0);
     return e;
-}
-
-// The persistent launch of the fused step: periodic grids without drive, and only when asked for (step_persist = 1).  Measured
-// slower than one launch per step replayed from a CUDA graph on every BASELINE workload (same run, Gcell*step/s: 1024^2 fp32
-// 51 against 111, 4096^2 fp32 181 against 211, cfg3 117 against 146, 16384^2 spinor 71 against 82; one 64^2 grid 3.9 against
-// 3.6 us per step): between steps a warp pays a fence, a release store, the neighbours' acquire polls and the refill of its
-// row pipeline, the state has to be read through L2 (ld.global.cg) instead of the non-coherent path, and the step loop costs
-// registers the row loop needs (spills).  DESIGN.md section 5.2.
-bool persist_wanted(const phx_grid* g) {
-    if (g->step_persist != 1 || g->persist_failed) return false;
-    return !(g->d.bc_x || g->d.bc_y || g->hasE || step_bulk(g));
 }
 
 int kernels_per_step(const phx_grid* g) {
@@ -840,8 +792,6 @@ phx_status phx_create_grid(phx_grid** out, const phx_grid_desc* desc) {
     g->step_bulk = -1;
     g->step_xch = -1;
     g->step_side = -1;
-    g->step_persist = -1;
-    g->persist_failed = false;
     g->step_warps = 0;
     g->async_host = 0;
     g->n_sm = prop.multiProcessorCount;
@@ -973,30 +923,8 @@ phx_status phx_step_rk4(phx_grid* g, int64_t n_steps) {
         }
         return PHX_OK;
     }
-    if (g->variant == PHX_VARIANT_STEP && n_steps >= 2 && persist_wanted(g)) {
-        int64_t left = n_steps;
-        while (left > 0) {
-            const int chunk = left > (1 << 20) ? (1 << 20) : (int)left;
-            const cudaError_t e = g->d.prec == PHX_C64 ? enqueue_step_fused<double>(g, g->stream, g->parity, chunk)
-                                                       : enqueue_step_fused<float>(g, g->stream, g->parity, chunk);
-            if (e == cudaErrorCooperativeLaunchTooLarge) {      // not all tiles resident: the graphs of single-step launches instead
-                cudaGetLastError();
-                g->persist_failed = true;
-                break;
-            }
-            PHX_CUDA(g, e);
-            g->parity ^= chunk & 1;
-            g->step_host += (uint64_t)chunk;
-            g->launches += 1;
-            left -= chunk;
-        }
-        if (left == 0) return PHX_OK;
-        n_steps = left;
-    }
     if (!g->graphs_valid) {
-        const bool refused = g->persist_failed;
         drop_graphs(g);
-        g->persist_failed = refused;
         PHX_CUDA(g, capture(g, 1, 0, &g->g1[0]));
         if (g->variant == PHX_VARIANT_STEP) PHX_CUDA(g, capture(g, 1, 1, &g->g1[1]));
         // the multi-step graph of the ping-pong variant must return to parity 0: an even number of steps
@@ -1205,9 +1133,6 @@ phx_status phx_set_tuning(phx_grid* g, const char* key, int32_t value) {
     } else if (!std::strcmp(key, "step_side")) {      // variant STEP side launch for a ragged last strip: 1 on; -1 (automatic) and 0: off
         if (value < -1 || value > 1) return PHX_ERR_INVALID_ARG;
         g->step_side = value;
-    } else if (!std::strcmp(key, "step_persist")) {   // variant STEP persistent launch: 1 on; -1 (automatic) and 0: off
-        if (value < -1 || value > 1) return PHX_ERR_INVALID_ARG;
-        g->step_persist = value;
     } else if (!std::strcmp(key, "async_host_copies")) {   // 1: phx_set_field / phx_read_field with PHX_HOST do not synchronise
         if (value != 0 && value != 1) return PHX_ERR_INVALID_ARG;
         g->async_host = value;

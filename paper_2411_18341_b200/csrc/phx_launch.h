@@ -78,21 +78,6 @@ PHX_DECL_STEP(32, float)
 PHX_DECL_STEP(64, double)
 #undef PHX_DECL_STEP
 
-// the persistent launch of the fused step (phx_step_inst.cu compiled with -DPHX_INST_PERS=1): a.n_steps steps in one cooperative
-// launch; periodic boundaries, no drive (zbc and bulk must be false); cudaErrorCooperativeLaunchTooLarge if the grid is not resident
-#define PHX_DECL_STEPP(P, T)                                                                                      \
-    cudaError_t launch_stepp_##P##_0(const StepArgs<T>&, bool noise, bool zbc, bool iso, bool bulk, int vec, dim3 grid, cudaStream_t); \
-    cudaError_t launch_stepp_##P##_1(const StepArgs<T>&, bool noise, bool zbc, bool iso, bool bulk, int vec, dim3 grid, cudaStream_t); \
-    cudaError_t launch_stepp_##P##_2(const StepArgs<T>&, bool noise, bool zbc, bool iso, bool bulk, int vec, dim3 grid, cudaStream_t); \
-    cudaError_t launch_stepp_##P##_3(const StepArgs<T>&, bool noise, bool zbc, bool iso, bool bulk, int vec, dim3 grid, cudaStream_t); \
-    int occupancy_stepp_##P##_0(bool noise, bool zbc, bool iso, bool drive, bool bulk, int vec);                                          \
-    int occupancy_stepp_##P##_1(bool noise, bool zbc, bool iso, bool drive, bool bulk, int vec);                                          \
-    int occupancy_stepp_##P##_2(bool noise, bool zbc, bool iso, bool drive, bool bulk, int vec);                                          \
-    int occupancy_stepp_##P##_3(bool noise, bool zbc, bool iso, bool drive, bool bulk, int vec);
-PHX_DECL_STEPP(32, float)
-PHX_DECL_STEPP(64, double)
-#undef PHX_DECL_STEPP
-
 // phx_stepx_inst.cu: the fused step with exchanging strips (scalar and reservoir models, periodic, no drive).  `vec` must be
 // one the precision and model have (stepx_has_vec); the CTA has a.wpc warps; occupancy = resident CTAs of `warps` warps per SM.
 #define PHX_DECL_STEPX(P, T)                                                                                  \
@@ -103,14 +88,6 @@ PHX_DECL_STEPP(64, double)
 PHX_DECL_STEPX(32, float)
 PHX_DECL_STEPX(64, double)
 #undef PHX_DECL_STEPX
-#define PHX_DECL_STEPXP(P, T)                                                                                  \
-    cudaError_t launch_stepxp_##P##_0(const StepArgs<T>&, bool noise, bool iso, int vec, dim3 grid, cudaStream_t); \
-    cudaError_t launch_stepxp_##P##_1(const StepArgs<T>&, bool noise, bool iso, int vec, dim3 grid, cudaStream_t); \
-    int occupancy_stepxp_##P##_0(bool noise, bool iso, int vec, int warps);                                        \
-    int occupancy_stepxp_##P##_1(bool noise, bool iso, int vec, int warps);
-PHX_DECL_STEPXP(32, float)
-PHX_DECL_STEPXP(64, double)
-#undef PHX_DECL_STEPXP
 // cells per lane the exchanging strips are instantiated with: complex fp32 2 (scalar also 4), complex fp64 1 (scalar also 2)
 inline bool stepx_has_vec(int prec64, int model, int vec) {
     if (model > 1) return false;

@@ -54,30 +54,23 @@ struct StepArgs {
     int strips;                 // strips per row of the grid
     int wpc;                    // warps per CTA of this launch (1 .. PHX_STEP_WARPS; the warps of a CTA are independent)
     int x0;                     // first output column of strip 0 (0, except in the side launch that covers a ragged last strip)
-    // persistent launch (template switch PERS): n_steps RK4 steps in ONE cooperative launch
-    int n_steps;
-    uint64_t step0;             // completed steps before this launch (the host's count; the device slots are written at the end)
-    uint32_t* flags;            // [batch][chunks][strips]: steps of this launch the tile has finished (zeroed before the launch)
 };
 
 namespace stepk {
 
-// CG: the array is rewritten by other SMs during the launch (persistent kernel): load through L2 (ld.global.cg), not through
-// the non-coherent path, whose L1 lines may date from two steps ago.
-template <bool CG, typename Q> __device__ __forceinline__ Q ldx(const Q* p) { return CG ? __ldcg(p) : __ldg(p); }
-template <int VEC, bool CG = false> __device__ __forceinline__ void ldc(const float2* p, float2 (&v)[VEC]) {
+template <int VEC> __device__ __forceinline__ void ldc(const float2* p, float2 (&v)[VEC]) {
     if constexpr (VEC % 2 == 0) {
 #pragma unroll
         for (int h = 0; h < VEC / 2; ++h) {
-            const float4 q = ldx<CG>(reinterpret_cast<const float4*>(p) + h);
+            const float4 q = __ldg(reinterpret_cast<const float4*>(p) + h);
             v[2 * h] = make_float2(q.x, q.y);
             v[2 * h + 1] = make_float2(q.z, q.w);
         }
-    } else v[0] = ldx<CG>(p);
+    } else v[0] = __ldg(p);
 }
-template <int VEC, bool CG = false> __device__ __forceinline__ void ldc(const double2* p, double2 (&v)[VEC]) {
+template <int VEC> __device__ __forceinline__ void ldc(const double2* p, double2 (&v)[VEC]) {
 #pragma unroll
-    for (int i = 0; i < VEC; ++i) v[i] = ldx<CG>(p + i);
+    for (int i = 0; i < VEC; ++i) v[i] = __ldg(p + i);
 }
 template <int VEC> __device__ __forceinline__ void stc(float2* p, const float2 (&v)[VEC]) {
     if constexpr (VEC % 2 == 0) {
@@ -89,14 +82,14 @@ template <int VEC> __device__ __forceinline__ void stc(double2* p, const double2
 #pragma unroll
     for (int i = 0; i < VEC; ++i) p[i] = v[i];
 }
-template <int VEC, bool CG = false> __device__ __forceinline__ void ldr(const float* p, float (&v)[VEC]) {
-    if constexpr (VEC == 4) { const float4 q = ldx<CG>(reinterpret_cast<const float4*>(p)); v[0] = q.x; v[1] = q.y; v[2] = q.z; v[3] = q.w; }
-    else if constexpr (VEC == 2) { const float2 q = ldx<CG>(reinterpret_cast<const float2*>(p)); v[0] = q.x; v[1] = q.y; }
-    else v[0] = ldx<CG>(p);
+template <int VEC> __device__ __forceinline__ void ldr(const float* p, float (&v)[VEC]) {
+    if constexpr (VEC == 4) { const float4 q = __ldg(reinterpret_cast<const float4*>(p)); v[0] = q.x; v[1] = q.y; v[2] = q.z; v[3] = q.w; }
+    else if constexpr (VEC == 2) { const float2 q = __ldg(reinterpret_cast<const float2*>(p)); v[0] = q.x; v[1] = q.y; }
+    else v[0] = __ldg(p);
 }
-template <int VEC, bool CG = false> __device__ __forceinline__ void ldr(const double* p, double (&v)[VEC]) {
-    if constexpr (VEC == 2) { const double2 q = ldx<CG>(reinterpret_cast<const double2*>(p)); v[0] = q.x; v[1] = q.y; }
-    else v[0] = ldx<CG>(p);
+template <int VEC> __device__ __forceinline__ void ldr(const double* p, double (&v)[VEC]) {
+    if constexpr (VEC == 2) { const double2 q = __ldg(reinterpret_cast<const double2*>(p)); v[0] = q.x; v[1] = q.y; }
+    else v[0] = __ldg(p);
 }
 template <int VEC> __device__ __forceinline__ void str(float* p, const float (&v)[VEC]) {
     if constexpr (VEC == 4) *reinterpret_cast<float4*>(p) = make_float4(v[0], v[1], v[2], v[3]);
@@ -179,36 +172,6 @@ __device__ __forceinline__ float2 xld(const float2* p) { float2 v; asm volatile(
 __device__ __forceinline__ double2 xld(const double2* p) { double2 v; asm volatile("ld.volatile.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(smem_u32(p))); return v; }
 __device__ __forceinline__ void xst_flag(int* p, int v) { asm volatile("st.volatile.shared.s32 [%0], %1;" ::"r"(smem_u32(p)), "r"(v)); }
 __device__ __forceinline__ int xld_flag(const int* p) { int v; asm volatile("ld.volatile.shared.s32 %0, [%1];" : "=r"(v) : "r"(smem_u32(p))); return v; }
-
-// ---- persistent launch (template switch PERS): a warp's tile (strip, chunk, realisation) may start step s of the launch once
-// every tile whose rows or columns it reads (and whose halo reads cover the cells it is about to overwrite) has finished step
-// s-1: the 5 x 5 tiles around it, wrapped (two on either side, so that a ragged last strip or chunk of fewer than 4 cells is
-// covered).  One lane per neighbour polls its counter with ld.acquire.gpu; a counter that does not arrive within seconds traps
-// (cannot happen under a cooperative launch, where all tiles are resident; the guard turns a hang into an error).
-__device__ __forceinline__ void pers_wait(const uint32_t* flags, int strips, int chunks, int strip, int chunk, int real, int lane,
-                                          uint32_t need) {
-    if (lane < 25) {
-        int sx = (strip + lane % 5 - 2) % strips, cy = (chunk + lane / 5 - 2) % chunks;
-        if (sx < 0) sx += strips;
-        if (cy < 0) cy += chunks;
-        const uint32_t* f = flags + ((size_t)real * chunks + cy) * strips + sx;
-        uint32_t v, spins = 0;
-        for (;;) {
-            asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(f) : "memory");
-            if (v >= need) break;
-            if (++spins > (1u << 22)) __trap();
-        }
-    }
-    __syncwarp();
-}
-__device__ __forceinline__ void pers_signal(uint32_t* flags, int strips, int chunks, int strip, int chunk, int real, int lane,
-                                            uint32_t done) {
-    __syncwarp();
-    if (lane == 0) {
-        __threadfence();
-        asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(flags + ((size_t)real * chunks + chunk) * strips + strip), "r"(done) : "memory");
-    }
-}
 
 // DRAM -> L2 prefetch of the line holding p (no register is tied up; the register fetch one row ahead then hits L2).
 __device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
@@ -293,13 +256,10 @@ struct StepSmem {
 // iteration j-1 and left in slot (j-1) & 1 of a two-slot ring; a warp enters iteration j once both neighbours have finished
 // j-1 (a progress counter per warp, polled in shared memory), so the warps of a row drift by less than one iteration and two
 // slots suffice.  Scalar and reservoir models (the TE-TM corners would need a neighbour's row of the SAME iteration), periodic.
-// PERS: a.n_steps RK4 steps in one cooperative launch; every warp keeps its tile and waits, between steps, only for the tiles
-// around it (pers_wait above) instead of for the whole grid: no launch, ramp and tail per step.  psi_in / psi_out (n_in /
-// n_out) swap roles every step; they are read through L2 (other SMs rewrite them during the launch).  Periodic, no drive.
 // UNITH: hbar = 1 exactly, so that 1/hbar times the potential is the potential (phx_deriv.cuh): one FP32 instruction fewer per
 // cell and stage of the 17 the scalar model issues.
 template <typename T, int VEC, int MODEL, bool NOISE, bool ZBC, bool ISO, bool DRIVE, int MINW, bool BULK, bool XCH = false,
-          bool PERS = false, bool UNITH = false>
+          bool UNITH = false>
 __global__ void __launch_bounds__(XCH ? 32 * PHX_STEP_XWARPS : 32 * PHX_STEP_WARPS, XCH ? 1 : MINW / PHX_STEP_WARPS)
 step_kernel(const __grid_constant__ StepArgs<T> a) {
     using namespace stepk;
@@ -311,18 +271,14 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
     constexpr int LEAD = XCH ? PHX_STEP_XLEAD : PHX_STEP_LEAD, RING = 4 + LEAD;
     static_assert(!(BULK && ZBC), "the bulk-copy fetch path is built for periodic boundaries");
     static_assert(!(XCH && (BULK || ZBC || SPINOR)), "the exchanging strips are built for periodic scalar / reservoir grids");
-    static_assert(!(PERS && (BULK || ZBC || DRIVE)), "the persistent launch is built for periodic grids without drive");
     const Geom& g = a.geo;
     const Coef<T>& k = a.k;
     const int nx = g.nx, ny = g.ny;
 
     const int lane = threadIdx.x & 31;
     const int strip = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
-    const uint64_t step0 = PERS ? a.step0 : *a.step_in;
-    if (blockIdx.x == 0 && blockIdx.y == 0 && blockIdx.z == 0 && threadIdx.x == 0 && a.x0 == 0) {
-        if (PERS) { const uint64_t after = step0 + (uint64_t)a.n_steps; *const_cast<uint64_t*>(a.step_in) = after; *a.step_out = after; }
-        else *a.step_out = step0 + 1;
-    }
+    const uint64_t step = *a.step_in;
+    if (blockIdx.x == 0 && blockIdx.y == 0 && blockIdx.z == 0 && threadIdx.x == 0 && a.x0 == 0) *a.step_out = step + 1;
     if (!XCH && strip >= a.strips) return;   // warp-uniform
     // exchanging strips: the ring of edge cells [2 slots][4 arrays: psi, y2, y3, y4][warp][side: 0 = first cell, 1 = last cell of
     // the strip] and the progress counters (front row of the last iteration a warp has finished)
@@ -354,16 +310,6 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
     const size_t boff = (size_t)blockIdx.z * g.plane;
     const bool zy = ZBC && g.bc_y;
 
-    // ---- the steps of this launch (one, unless PERS) ---------------------------------------------------------------------------
-#pragma unroll 1
-    for (int it = 0; it < (PERS ? a.n_steps : 1); ++it) {
-    const uint64_t step = step0 + (uint64_t)it;
-    const bool swapped = PERS && (it & 1);      // odd steps of a persistent launch read what the even ones wrote
-    const int xkey = PERS ? it * (a.ly + 16) : 0;   // (XCH) keeps the warps' progress counters monotonic from step to step
-    if constexpr (PERS) {
-        if (it > 0) pers_wait(a.flags, a.strips, (int)gridDim.y, strip, (int)blockIdx.y, (int)blockIdx.z, lane, (uint32_t)it);
-    }
-
     // drive: q_s = (1/hbar) exp(-i omega t_s) at the stage times t, t + dt/2, t + dt, t = step dt; the phase is evaluated
     // in double and rounded to T (reading Q17)
     C q1 = mk<T>(T(0), T(0)), q23 = q1, q4 = q1;
@@ -383,10 +329,10 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
     T* nout_p[NC];
 #pragma unroll
     for (int s = 0; s < NC; ++s) {
-        pin[s] = (swapped ? a.psi_out[s] : a.psi_in[s]) + boff;
-        pout[s] = (swapped ? const_cast<C*>(a.psi_in[s]) : a.psi_out[s]) + boff;
-        nin[s] = RES ? (swapped ? a.n_out[s] : a.n_in[s]) + boff : nullptr;
-        nout_p[s] = RES ? (swapped ? const_cast<T*>(a.n_in[s]) : a.n_out[s]) + boff : nullptr;
+        pin[s] = a.psi_in[s] + boff;
+        pout[s] = a.psi_out[s] + boff;
+        nin[s] = RES ? a.n_in[s] + boff : nullptr;
+        nout_p[s] = RES ? a.n_out[s] + boff : nullptr;
     }
     const T* Vp = a.V;
     const T* Pp = RES ? a.P : nullptr;
@@ -465,7 +411,7 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
         const bool okq = !ZBC || (inx && (!zy || (qw >= 0 && qw < ny)));
 #pragma unroll
         for (int s = 0; s < NC; ++s) {
-            if (okq) ldc<VEC, PERS>(pin[s] + ew, psr[s][(d + R2) % RING]);
+            if (okq) ldc<VEC>(pin[s] + ew, psr[s][(d + R2) % RING]);
         }
         if (d >= 0 && d < LEAD && okq) {
             if (Vp) ldr<VEC>(Vp + ew, Vr[(d + R2) % RING]);
@@ -473,7 +419,7 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
             if (DRIVE) ldc<VEC>(Ep + ew, Er[(d + R2) % RING]);
             if constexpr (RES) {
 #pragma unroll
-                for (int s = 0; s < NC; ++s) ldr<VEC, PERS>(nin[s] + ew, nr[s][(d + R2) % RING]);
+                for (int s = 0; s < NC; ++s) ldr<VEC>(nin[s] + ew, nr[s][(d + R2) % RING]);
             }
         }
         ewp = ew;
@@ -496,7 +442,7 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
 #if PHX_XCH_SYNC == 1
         __syncthreads();
 #else
-        if (lane == 0) xst_flag(xp + strip, j0 - 1 + xkey);
+        if (lane == 0) xst_flag(xp + strip, j0 - 1);
 #endif
     }
 
@@ -577,7 +523,7 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
             C xin[4];                       // (XCH) the neighbours' cells next to this lane's strip: of psi[j], y2[j-1], y3[j-2], y4[j-3]
             if constexpr (XCH) {
 #if PHX_XCH_SYNC == 0
-                while (xld_flag(xp + xleft) < j - 1 + xkey || xld_flag(xp + xright) < j - 1 + xkey) { }   // both finished iteration j-1
+                while (xld_flag(xp + xleft) < j - 1 || xld_flag(xp + xright) < j - 1) { }   // both finished iteration j-1
 #endif
 #pragma unroll
                 for (int q = 0; q < 4; ++q) xin[q] = xld(xe + (((j - 1) & 1) * 4 + q) * XARR + xrd);
@@ -643,7 +589,7 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
 #pragma unroll
                     for (int i = 0; i < VEC; ++i) psr[s][SL(1 + LEAD)][i] = czero;
                 }
-                if (okq) ldc<VEC, PERS>(pin[s] + ew, psr[s][SL(1 + LEAD)]);
+                if (okq) ldc<VEC>(pin[s] + ew, psr[s][SL(1 + LEAD)]);
             }
             if (ZBC) {              // (periodic without V or P: the slots keep the zeros they were initialised with)
 #pragma unroll
@@ -661,7 +607,7 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
 #pragma unroll
                         for (int i = 0; i < VEC; ++i) nr[s][SL(LEAD)][i] = T(0);
                     }
-                    if (okprev) ldr<VEC, PERS>(nin[s] + ewp, nr[s][SL(LEAD)]);
+                    if (okprev) ldr<VEC>(nin[s] + ewp, nr[s][SL(LEAD)]);
                 }
             }
             }
@@ -752,7 +698,7 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
 #if PHX_XCH_SYNC == 1
                     asm volatile("bar.sync 1, %0;" ::"r"((int)blockDim.x));   // iteration j's cells are out: the warps of the row step together
 #else
-                    if (lane == 0) xst_flag(xp + strip, j + xkey);                             // iteration j's cells are out
+                    if (lane == 0) xst_flag(xp + strip, j);                             // iteration j's cells are out
 #endif
                 }
 
@@ -809,8 +755,6 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
             if (!zy && qw == ny) { qw = 0; ew -= plane; }
         }
     }
-    if constexpr (PERS) pers_signal(a.flags, a.strips, (int)gridDim.y, strip, (int)blockIdx.y, (int)blockIdx.z, lane, (uint32_t)(it + 1));
-    }   // steps of this launch
 #undef SL
 }
 

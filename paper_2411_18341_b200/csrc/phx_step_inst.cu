@@ -6,11 +6,6 @@
 #ifndef PHX_INST_PREC
 #error "compile with -DPHX_INST_PREC=32|64 -DPHX_INST_MODEL=0..3"
 #endif
-// -DPHX_INST_PERS=1: the same file instantiates the PERSISTENT launch (phx_step.cuh, PERS: all steps of a call in one
-// cooperative launch; periodic boundaries, no drive, register loads) under the names launch_stepp_* / occupancy_stepp_*.
-#ifndef PHX_INST_PERS
-#define PHX_INST_PERS 0
-#endif
 
 namespace phx {
 
@@ -19,6 +14,7 @@ typedef float real_t;
 #else
 typedef double real_t;
 #endif
+
 
 // Resident warps per SM the register budget is sized for: the carried register rings grow with the number of
 // components and reservoirs (DESIGN.md section 5.2 has the count per model).
@@ -53,7 +49,7 @@ struct Inst {
     static constexpr bool I = ISO && PHX_HAS_ISO;
     // dynamic shared memory: the per-warp rings of the bulk-copy fetch path
     static constexpr size_t SMEM = BULK ? StepSmem<real_t, VEC, PHX_INST_MODEL, DRIVE>::CTA : 0;
-    static auto kernel() { return step_kernel<real_t, VEC, PHX_INST_MODEL, NOISE, ZBC, I, DRIVE, MINW, BULK, false, PHX_INST_PERS != 0, UNITH>; }
+    static auto kernel() { return step_kernel<real_t, VEC, PHX_INST_MODEL, NOISE, ZBC, I, DRIVE, MINW, BULK, false, UNITH>; }
     static cudaError_t prepare() {
         if (SMEM > 48 * 1024) {
             static cudaError_t once = cudaFuncSetAttribute(kernel(), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM);
@@ -64,14 +60,8 @@ struct Inst {
     static cudaError_t launch(const StepArgs<real_t>& a, dim3 grid, cudaStream_t st) {
         cudaError_t e = prepare();
         if (e != cudaSuccess) return e;
-#if PHX_INST_PERS
-        // cooperative: every CTA of the grid is resident, or the launch fails (cudaErrorCooperativeLaunchTooLarge)
-        void* args[] = {const_cast<StepArgs<real_t>*>(&a)};
-        return cudaLaunchCooperativeKernel((const void*)kernel(), grid, dim3(32 * a.wpc), args, SMEM, st);
-#else
         kernel()<<<grid, 32 * a.wpc, SMEM, st>>>(a);
         return cudaGetLastError();
-#endif
     }
     static int occupancy() {   // resident CTAs of PHX_STEP_WARPS warps per SM (the register file bounds the WARPS)
         int nb = 0;
@@ -89,23 +79,16 @@ struct Inst {
 // multiply by 1.0f -- the same bits.
 template <int VEC, bool NOISE, bool DRIVE, typename F>
 static auto dispatch2(bool zbc, bool iso, bool bulk, bool unith, F f) {
-#if PHX_INST_PERS
-    return iso ? f(Inst<VEC, NOISE, false, true, false, false>()) : f(Inst<VEC, NOISE, false, false, false, false>());
-#else
     if (zbc) return iso ? f(Inst<VEC, NOISE, true, true, DRIVE, false>()) : f(Inst<VEC, NOISE, true, false, DRIVE, false>());
     if (bulk) return iso ? f(Inst<VEC, NOISE, false, true, DRIVE, true>()) : f(Inst<VEC, NOISE, false, false, DRIVE, true>());
     if constexpr (!DRIVE) {
         if (unith && iso) return f(Inst<VEC, NOISE, false, true, false, false, true>());
     }
     return iso ? f(Inst<VEC, NOISE, false, true, DRIVE, false>()) : f(Inst<VEC, NOISE, false, false, DRIVE, false>());
-#endif
 }
 
 template <int VEC, typename F>
 static auto dispatch(bool noise, bool zbc, bool iso, bool drive, bool bulk, bool unith, F f) {
-#if PHX_INST_PERS
-    return noise ? dispatch2<VEC, true, false>(false, iso, false, false, f) : dispatch2<VEC, false, false>(false, iso, false, false, f);
-#endif
     if (noise && drive) return dispatch2<VEC, true, true>(zbc, iso, bulk, unith, f);   // Eq. (16) carries E and dW together
     if (noise) return dispatch2<VEC, true, false>(zbc, iso, bulk, unith, f);
     if (drive) return dispatch2<VEC, false, true>(zbc, iso, bulk, unith, f);
@@ -123,17 +106,10 @@ static cudaError_t launch_vec(const StepArgs<real_t>& a, bool noise, bool zbc, b
 }
 
 #define PHX_CAT3(a, b, c) a##b##_##c
-#if PHX_INST_PERS
-#define PHX_NAME(p, m) PHX_CAT3(launch_stepp_, p, m)
-#else
 #define PHX_NAME(p, m) PHX_CAT3(launch_step_, p, m)
-#endif
 
 cudaError_t PHX_NAME(PHX_INST_PREC, PHX_INST_MODEL)(const StepArgs<real_t>& a, bool noise, bool zbc, bool iso, bool bulk, int vec,
                                                     dim3 grid, cudaStream_t st) {
-#if PHX_INST_PERS
-    if (zbc || bulk || a.E != nullptr || a.n_steps < 1 || a.flags == nullptr) return cudaErrorInvalidValue;
-#endif
 #if PHX_INST_PREC == 32
 #if PHX_HAS_VEC4
     if (vec == 4) return launch_vec<4>(a, noise, zbc, iso, bulk, grid, st);
@@ -146,11 +122,7 @@ cudaError_t PHX_NAME(PHX_INST_PREC, PHX_INST_MODEL)(const StepArgs<real_t>& a, b
     return cudaErrorInvalidValue;
 }
 
-#if PHX_INST_PERS
-#define PHX_OCC_NAME(p, m) PHX_CAT3(occupancy_stepp_, p, m)
-#else
 #define PHX_OCC_NAME(p, m) PHX_CAT3(occupancy_step_, p, m)
-#endif
 
 // Resident CTAs per SM of the instantiation (for the launch plan: one balanced wave).
 int PHX_OCC_NAME(PHX_INST_PREC, PHX_INST_MODEL)(bool noise, bool zbc, bool iso, bool drive, bool bulk, int vec) {

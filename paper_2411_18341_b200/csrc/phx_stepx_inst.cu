@@ -6,10 +6,6 @@
 #ifndef PHX_INST_PREC
 #error "compile with -DPHX_INST_PREC=32|64 -DPHX_INST_MODEL=0|1"
 #endif
-// -DPHX_INST_PERS=1: the persistent launch of the same kernels (launch_stepxp_* / occupancy_stepxp_*).
-#ifndef PHX_INST_PERS
-#define PHX_INST_PERS 0
-#endif
 
 namespace phx {
 
@@ -19,17 +15,13 @@ typedef float real_t;
 typedef double real_t;
 #endif
 
+
 template <int VEC, bool NOISE, bool ISO>
 struct InstX {
-    static auto kernel() { return step_kernel<real_t, VEC, PHX_INST_MODEL, NOISE, false, ISO, false, 8, false, true, PHX_INST_PERS != 0>; }
+    static auto kernel() { return step_kernel<real_t, VEC, PHX_INST_MODEL, NOISE, false, ISO, false, 8, false, true>; }
     static cudaError_t launch(const StepArgs<real_t>& a, dim3 grid, cudaStream_t st) {
-#if PHX_INST_PERS
-        void* args[] = {const_cast<StepArgs<real_t>*>(&a)};
-        return cudaLaunchCooperativeKernel((const void*)kernel(), grid, dim3(32 * a.wpc), args, 0, st);
-#else
         kernel()<<<grid, 32 * a.wpc, 0, st>>>(a);
         return cudaGetLastError();
-#endif
     }
     static int occupancy(int warps) {
         int nb = 0;
@@ -56,19 +48,11 @@ static auto dispatchx(bool noise, bool iso, F f) {
 #endif
 
 #define PHX_CAT3(a, b, c) a##b##_##c
-#if PHX_INST_PERS
-#define PHX_NAME(p, m) PHX_CAT3(launch_stepxp_, p, m)
-#define PHX_OCC_NAME(p, m) PHX_CAT3(occupancy_stepxp_, p, m)
-#else
 #define PHX_NAME(p, m) PHX_CAT3(launch_stepx_, p, m)
 #define PHX_OCC_NAME(p, m) PHX_CAT3(occupancy_stepx_, p, m)
-#endif
 
 cudaError_t PHX_NAME(PHX_INST_PREC, PHX_INST_MODEL)(const StepArgs<real_t>& a, bool noise, bool iso, int vec, dim3 grid, cudaStream_t st) {
     if (a.wpc < 1 || a.wpc > PHX_STEP_XWARPS || a.E != nullptr) return cudaErrorInvalidValue;
-#if PHX_INST_PERS
-    if (a.n_steps < 1 || a.flags == nullptr) return cudaErrorInvalidValue;
-#endif
     if (vec == PHX_XVEC_A) return dispatchx<PHX_XVEC_A>(noise, iso, [&](auto inst) { return decltype(inst)::launch(a, grid, st); });
 #if PHX_INST_MODEL == 0
     if (vec == PHX_XVEC_B) return dispatchx<PHX_XVEC_B>(noise, iso, [&](auto inst) { return decltype(inst)::launch(a, grid, st); });

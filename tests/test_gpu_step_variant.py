@@ -209,7 +209,7 @@ def test_spinor_noise():
     run_pair(w, 30)
 
 
-# ---- exchanging strips (the warps of a CTA tile the whole row) and the persistent launch -------------------
+# ---- exchanging strips (the warps of a CTA tile the whole row), side launch, bulk-copy fetch ---------------
 def _fields(g, w):
     return {name: g.read_field(name) for name in w.fields}
 
@@ -258,33 +258,6 @@ def test_exchanging_strips_are_the_default_for_ensembles_of_narrow_grids():
     ref.step_rk4(7)
     for name in w.fields:
         assert np.array_equal(g.read_field(name), ref.read_field(name)), name
-    g.destroy()
-    ref.destroy()
-
-
-@pytest.mark.parametrize("maker,tuning", [
-    (lambda: wl.cfg2(n=300, ny=70, prec="c32"), {}), (lambda: wl.cfg2(n=200, ny=64, prec="c64"), {"step_ly": 9}),
-    (lambda: wl.cfg3(n=160, prec="c32"), {"step_ly": 23}), (lambda: wl.cfg4(n=120, prec="c32", sigma_cells=10.0), {}),
-    (lambda: wl.cfg5(n=64, batch=5, prec="c32"), {}), (lambda: wl.cfg5(n=128, batch=3, prec="c32"), {"step_xch": 1}),
-    (lambda: wl.cfg2(n=2048, ny=40, prec="c32"), {"step_ly": 8})])
-def test_persistent_launch(maker, tuning):
-    # step_persist = 1: all steps of a call in ONE cooperative launch, the tiles synchronised by neighbour flags; against the
-    # oracle, bit for bit against one launch per step, odd and even step counts, and continued by ordinary steps
-    w = maker()
-    g = make_gpu(w, variant=STEP, tuning=dict(tuning, step_persist=1))
-    ref = make_gpu(w, variant=STEP, tuning=tuning)
-    o = make_oracle(w)
-    g.step_rk4(21)
-    assert g.get_launch_count() == 1
-    g.step_rk4(10)
-    assert g.get_launch_count() == 2
-    g.step_rk4(1)                                   # a single step takes the ordinary launch
-    ref.step_rk4(32)
-    o.step_rk4(32)
-    compare(g, o, w)
-    for name in w.fields:
-        assert np.array_equal(g.read_field(name), ref.read_field(name)), name
-    assert g.get_step() == 32
     g.destroy()
     ref.destroy()
 

@@ -20,7 +20,7 @@ typedef double real_t;
 // components and reservoirs (DESIGN.md section 5.2 has the count per model).
 #if PHX_INST_PREC == 32
 #ifndef PHX_MINW_V2
-#define PHX_MINW_V2 (PHX_INST_MODEL == 0 ? 16 : (PHX_INST_MODEL == 1 ? 12 : 8))
+#define PHX_MINW_V2 (PHX_INST_MODEL == 0 ? 16 : 8)   // (reservoir, cfg3: 143.5 Gcell*step/s with the registers of 8 resident warps, 140.7 with 12, 132 with 16)
 #endif
 #define PHX_MINW_V1 (PHX_INST_MODEL == 0 ? 24 : (PHX_INST_MODEL == 1 ? 20 : 12))
 #else
@@ -44,8 +44,7 @@ typedef double real_t;
 
 template <int VEC, bool NOISE, bool ZBC, bool ISO, bool DRIVE, bool BULK, bool UNITH = false>
 struct Inst {
-    // (the noisy reservoir kernel, cfg5, is 9 % faster with the registers of 8 resident warps than with those of 12)
-    static constexpr int MINW = VEC == 4 ? PHX_MINW_V4 : (VEC == 2 ? ((NOISE && PHX_INST_MODEL == 1 && PHX_INST_PREC == 32) ? 8 : PHX_MINW_V2) : PHX_MINW_V1);
+    static constexpr int MINW = VEC == 4 ? PHX_MINW_V4 : (VEC == 2 ? PHX_MINW_V2 : PHX_MINW_V1);
     static constexpr bool I = ISO && PHX_HAS_ISO;
     // dynamic shared memory: the per-warp rings of the bulk-copy fetch path
     static constexpr size_t SMEM = BULK ? StepSmem<real_t, VEC, PHX_INST_MODEL, DRIVE>::CTA : 0;

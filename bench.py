@@ -43,6 +43,8 @@ def build_workload(name, quick=False):
         "cfg1": lambda: wl.cfg1(),
         "cfg2_1024_c32": lambda: wl.cfg2(1024, "c32"), "cfg2_1024_c64": lambda: wl.cfg2(1024, "c64"),
         "cfg2_4096_c32": lambda: wl.cfg2(4096, "c32"), "cfg2_4096_c64": lambda: wl.cfg2(4096, "c64"),
+        # beyond BASELINE's sizes (the scalar model on larger grids: the fused step's rate away from single-wave effects)
+        "cfg2_8192_c32": lambda: wl.cfg2(8192, "c32", tile=2048), "cfg2_16384_c32": lambda: wl.cfg2(16384, "c32", tile=2048),
         "cfg3_4096_c32": lambda: wl.cfg3(4096, "c32"),
         "cfg4_16384_c32": lambda: wl.cfg4(16384, "c32"), "cfg4_8192_c32": lambda: wl.cfg4(8192, "c32"),
         "cfg5_512x256_c32": lambda: wl.cfg5(256, 512, "c32"),
@@ -447,15 +449,15 @@ def main():
         g.destroy()
         del g
         torch.cuda.empty_cache()
-        for name in ("cfg2_4096_c64", "cfg3_4096_c32", "cfg5_512x256_c32", "cfg4_16384_c32", "cfg2_1024_c32"):
+        for name in ("cfg2_4096_c64", "cfg3_4096_c32", "cfg5_512x256_c32", "cfg4_16384_c32", "cfg2_1024_c32", "cfg2_16384_c32"):
             ow = build_workload(name, quick=True)
             og = phx.grid_from_workload(ow, stream=stream, device=f"cuda:{local}")
             rec = {}
-            for vname, v in (("auto", phx.PHX_VARIANT_AUTO), ("stage", phx.PHX_VARIANT_STAGE)):
+            for vname, v in (("auto", phx.PHX_VARIANT_AUTO), ("stage", phx.PHX_VARIANT_STAGE))[:1 if name == "cfg2_16384_c32" else 2]:
                 og.select_variant(v)
                 vv = og.get_variant()
                 og.step_rk4(5)
-                o_steps = 16 if name.startswith("cfg4") else 64
+                o_steps = 16 if "16384" in name else 64
                 o_ms, o_l, o_nb, _ = timed_blocks(og, o_steps, 0.2)
                 val = ow.cells * o_steps / (o_ms * 1e-3) / 1e9
                 ob = algo_bytes_per_cell_step(ow, vv, o_steps)

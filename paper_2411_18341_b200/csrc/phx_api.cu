@@ -92,6 +92,7 @@ struct phx_grid {
     cudaStream_t side_stream;   // second branch of the captured step (the side launch of a ragged last strip)
     cudaEvent_t ev_fork, ev_join;
     int step_side;          // variant STEP side launch for a ragged last strip: 1 on; -1 and 0: off
+    int step_pdl;           // variant STEP: later steps of a graph as programmatic dependent launches: -1 automatic, 0 off, 1 on
     bool has_params;
     phx_params prm;
     double coef[PHX_NCOEF];
@@ -450,8 +451,9 @@ StepPlan step_plan(const phx_grid* g) {
 }
 
 // One RK4 step of variant STEP: a single kernel that reads the state of parity p and writes parity 1-p.
+// pdl: launch as a programmatic dependent of the previous kernel in the stream (the later steps of a captured graph)
 template <typename T>
-cudaError_t enqueue_step_fused(phx_grid* g, cudaStream_t st, int parity) {
+cudaError_t enqueue_step_fused(phx_grid* g, cudaStream_t st, int parity, bool pdl = false) {
     using C = typename Cx<T>::type;
     StepArgs<T> a;
     std::memset(&a, 0, sizeof(a));
@@ -477,6 +479,7 @@ cudaError_t enqueue_step_fused(phx_grid* g, cudaStream_t st, int parity) {
     a.step_in = slots + parity;
     a.step_out = slots + (1 - parity);
     a.seed = g->prm.seed;
+    a.pdl = pdl ? 1 : 0;
     const StepPlan plan = step_plan(g);
     const int vec = plan.vec;
     a.strips = plan.xch ? plan.wpc : step_strips(g, vec);
@@ -510,6 +513,7 @@ cudaError_t enqueue_step_fused(phx_grid* g, cudaStream_t st, int parity) {
     };
     if (plan.side_cols == 0) return launch(a, vec, grid, st);
     // main launch (whole strips) and side launch (the remaining columns, one cell per lane) on two branches
+    a.pdl = 0;      // (events between the branches: ordinary dependencies)
     cudaError_t e = cudaEventRecord(g->ev_fork, st);
     if (e == cudaSuccess) e = cudaStreamWaitEvent(g->side_stream, g->ev_fork, 0);
     if (e == cudaSuccess) e = launch(a, vec, grid, st);
@@ -522,6 +526,16 @@ cudaError_t enqueue_step_fused(phx_grid* g, cudaStream_t st, int parity) {
     if (e == cudaSuccess) e = cudaEventRecord(g->ev_join, g->side_stream);
     if (e == cudaSuccess) e = cudaStreamWaitEvent(st, g->ev_join, 0);
     return e;
+}
+
+// Programmatic dependent launches inside a graph of fused steps (the CTAs of step s+1 are scheduled early and wait in
+// griddepcontrol.wait for step s): hides the launch latency, which is all a tiny grid has -- one 64^2 grid 3.33 against 3.58 us
+// per step, cfg1 3.59 against 3.84, 256^2 3.59 against 3.84 -- but CTAs that are placed while the previous grid still holds
+// most SMs end up unevenly spread: 512^2 -5 %, 1024^2 82 against 113 Gcell*step/s, 4096^2 -3 %.  Automatic: up to 256^2 cells.
+bool step_pdl_wanted(const phx_grid* g) {
+    if (g->step_pdl == 0 || g->variant != PHX_VARIANT_STEP) return false;
+    if (g->step_pdl == 1) return true;
+    return plane_cells(g) * g->d.batch <= (size_t)256 * 256;
 }
 
 int kernels_per_step(const phx_grid* g) {
@@ -550,9 +564,9 @@ cudaError_t launch_resident(phx_grid* g, int n_steps) {
 }
 
 // Enqueues one step starting from state parity `parity` (always 0 for variant STAGE).
-cudaError_t enqueue_step(phx_grid* g, cudaStream_t st, int parity) {
+cudaError_t enqueue_step(phx_grid* g, cudaStream_t st, int parity, bool pdl = false) {
     if (g->variant == PHX_VARIANT_STEP)
-        return g->d.prec == PHX_C64 ? enqueue_step_fused<double>(g, st, parity) : enqueue_step_fused<float>(g, st, parity);
+        return g->d.prec == PHX_C64 ? enqueue_step_fused<double>(g, st, parity, pdl) : enqueue_step_fused<float>(g, st, parity, pdl);
     return g->d.prec == PHX_C64 ? enqueue_step_stage<double>(g, st) : enqueue_step_stage<float>(g, st);
 }
 
@@ -562,7 +576,7 @@ cudaError_t capture(phx_grid* g, int steps, int parity, cudaGraphExec_t* out) {
     if (e != cudaSuccess) return e;
     cudaError_t le = cudaSuccess;
     for (int s = 0; s < steps && le == cudaSuccess; ++s) {
-        le = enqueue_step(g, g->cap_stream, parity);
+        le = enqueue_step(g, g->cap_stream, parity, s > 0 && step_pdl_wanted(g));
         if (g->variant == PHX_VARIANT_STEP) parity ^= 1;
     }
     e = cudaStreamEndCapture(g->cap_stream, &graph);
@@ -792,6 +806,7 @@ phx_status phx_create_grid(phx_grid** out, const phx_grid_desc* desc) {
     g->step_bulk = -1;
     g->step_xch = -1;
     g->step_side = -1;
+    g->step_pdl = -1;
     g->step_warps = 0;
     g->async_host = 0;
     g->n_sm = prop.multiProcessorCount;
@@ -1130,6 +1145,9 @@ phx_status phx_set_tuning(phx_grid* g, const char* key, int32_t value) {
     } else if (!std::strcmp(key, "step_xch")) {       // variant STEP exchanging strips: -1 automatic (wherever the row fits), 0 off
         if (value < -1 || value > 1) return PHX_ERR_INVALID_ARG;
         g->step_xch = value;
+    } else if (!std::strcmp(key, "step_pdl")) {       // variant STEP programmatic dependent launches inside a graph: -1 automatic, 0 off, 1 on
+        if (value < -1 || value > 1) return PHX_ERR_INVALID_ARG;
+        g->step_pdl = value;
     } else if (!std::strcmp(key, "step_side")) {      // variant STEP side launch for a ragged last strip: 1 on; -1 (automatic) and 0: off
         if (value < -1 || value > 1) return PHX_ERR_INVALID_ARG;
         g->step_side = value;

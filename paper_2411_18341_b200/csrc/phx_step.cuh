@@ -59,6 +59,7 @@ struct StepArgs {
     int strips;                 // strips per row of the grid
     int wpc;                    // warps per CTA of this launch (1 .. PHX_STEP_WARPS; the warps of a CTA are independent)
     int x0;                     // first output column of strip 0 (0, except in the side launch that covers a ragged last strip)
+    int pdl;                    // (host side) launch as a programmatic dependent of the previous kernel of the stream
 };
 
 namespace stepk {
@@ -292,6 +293,12 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
     const Coef<T>& k = a.k;
     const int nx = g.nx, ny = g.ny;
 
+    // Programmatic dependent launch (a.pdl, set by the host for the second and later steps of a captured graph): the CTAs of
+    // this grid may be scheduled while the previous step's grid is still running and wait here until it has completed and its
+    // writes are visible -- the launch latency between two steps is hidden, nothing else changes (every global access of this
+    // kernel, the step counter included, comes after the wait).  Both instructions do nothing in an ordinary launch.
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    asm volatile("griddepcontrol.wait;" ::: "memory");
     const int lane = threadIdx.x & 31;
     const int strip = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
     const uint64_t step = *a.step_in;

@@ -15,6 +15,23 @@ typedef float real_t;
 typedef double real_t;
 #endif
 
+// a.pdl: programmatic stream serialisation (the grid may be scheduled before the previous kernel of the stream has finished; it
+// waits in griddepcontrol.wait, phx_step.cuh)
+template <typename K>
+static cudaError_t launch_maybe_pdl(K kernel, const StepArgs<real_t>& a, dim3 grid, size_t smem, cudaStream_t st) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid;
+    cfg.blockDim = dim3(32 * a.wpc);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = a.pdl ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, kernel, a);
+}
+
 
 // Resident warps per SM the register budget is sized for: the carried register rings grow with the number of
 // components and reservoirs (DESIGN.md section 5.2 has the count per model).
@@ -59,8 +76,7 @@ struct Inst {
     static cudaError_t launch(const StepArgs<real_t>& a, dim3 grid, cudaStream_t st) {
         cudaError_t e = prepare();
         if (e != cudaSuccess) return e;
-        kernel()<<<grid, 32 * a.wpc, SMEM, st>>>(a);
-        return cudaGetLastError();
+        return launch_maybe_pdl(kernel(), a, grid, SMEM, st);
     }
     static int occupancy() {   // resident CTAs of PHX_STEP_WARPS warps per SM (the register file bounds the WARPS)
         int nb = 0;

@@ -15,13 +15,29 @@ typedef float real_t;
 typedef double real_t;
 #endif
 
+// a.pdl: programmatic stream serialisation (the grid may be scheduled before the previous kernel of the stream has finished; it
+// waits in griddepcontrol.wait, phx_step.cuh)
+template <typename K>
+static cudaError_t launch_maybe_pdl(K kernel, const StepArgs<real_t>& a, dim3 grid, size_t smem, cudaStream_t st) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid;
+    cfg.blockDim = dim3(32 * a.wpc);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = a.pdl ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, kernel, a);
+}
+
 
 template <int VEC, bool NOISE, bool ISO>
 struct InstX {
     static auto kernel() { return step_kernel<real_t, VEC, PHX_INST_MODEL, NOISE, false, ISO, false, 8, false, true>; }
     static cudaError_t launch(const StepArgs<real_t>& a, dim3 grid, cudaStream_t st) {
-        kernel()<<<grid, 32 * a.wpc, 0, st>>>(a);
-        return cudaGetLastError();
+        return launch_maybe_pdl(kernel(), a, grid, 0, st);
     }
     static int occupancy(int warps) {
         int nb = 0;

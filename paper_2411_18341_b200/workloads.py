@@ -94,8 +94,20 @@ def cfg1(n=64, prec="c64", n_steps=1000):
                     fields={"psi_p": psi[None]})
 
 
-def cfg2(n=4096, prec="c32", n_steps=10000, ny=None):
-    """Config 2: scalar Eq. (1), n x n (1024, 4096), smooth disorder V, uniform random psi0."""
+def cfg2(n=4096, prec="c32", n_steps=10000, ny=None, tile=None):
+    """Config 2: scalar Eq. (1), n x n (1024, 4096), smooth disorder V, uniform random psi0.
+
+    tile=t (t divides n, square grids): the recipe is drawn on a t x t grid and repeated periodically to n x n (the disorder is
+    periodic, so the tiling is seamless); used by bench.py for sizes beyond BASELINE's (8192^2, 16384^2), ready in seconds."""
+    if tile is not None and tile != n:
+        if n % tile != 0 or ny not in (None, n):
+            raise ValueError("tile must divide n (square grids)")
+        w = cfg2(tile, prec, n_steps)
+        reps = n // tile
+        w.V = np.tile(w.V, (reps, reps))
+        w.fields = {k: np.tile(v, (1, reps, reps)) for k, v in w.fields.items()}
+        w.name, w.nx, w.ny = f"cfg2_{n}x{n}_{prec}", n, n
+        return w
     dx = 0.2
     ny = n if ny is None else ny
     cdt, rdt = _CDT[prec], _RDT[prec]

@@ -262,6 +262,25 @@ def test_exchanging_strips_are_the_default_for_ensembles_of_narrow_grids():
     ref.destroy()
 
 
+@pytest.mark.parametrize("maker", [lambda: wl.cfg1(n_steps=60), lambda: wl.cfg2(n=300, ny=70, prec="c32"), lambda: wl.cfg3(n=160, prec="c32"),
+                                   lambda: wl.cfg4(n=120, prec="c32", sigma_cells=10.0), lambda: wl.cfg5(n=64, batch=5, prec="c32"),
+                                   lambda: wl.cfg2(n=1024, ny=256, prec="c32")])
+def test_programmatic_dependent_launches_give_the_same_bits(maker):
+    # step_pdl: the later steps of a captured graph are programmatic dependents of the step before (griddepcontrol.wait at the
+    # top of the kernel orders everything); forced on and off, odd and even step counts, noise counter included
+    w = maker()
+    on = make_gpu(w, variant=STEP, tuning={"step_pdl": 1})
+    off = make_gpu(w, variant=STEP, tuning={"step_pdl": 0})
+    for n in (19, 8, 1):
+        on.step_rk4(n)
+        off.step_rk4(n)
+    for name in w.fields:
+        assert np.array_equal(on.read_field(name), off.read_field(name)), name
+    assert on.get_step() == off.get_step() == 28
+    on.destroy()
+    off.destroy()
+
+
 @pytest.mark.parametrize("nx,bc,noise", [(2048, (0, 0), False), (2416, (0, 0), True), (4096, (0, 0), False), (2188, (1, 1), False),
                                          (2428, (0, 1), False)])
 def test_side_launch_for_a_ragged_last_strip(nx, bc, noise):

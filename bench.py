@@ -48,6 +48,8 @@ def build_workload(name, quick=False):
         "cfg3_4096_c32": lambda: wl.cfg3(4096, "c32"),
         "cfg4_16384_c32": lambda: wl.cfg4(16384, "c32"), "cfg4_8192_c32": lambda: wl.cfg4(8192, "c32"),
         "cfg5_512x256_c32": lambda: wl.cfg5(256, 512, "c32"),
+        # spinor with reservoirs (the paper's full 24-buffer system, Example 3) at its 500^2 and at a 4096^2 shape
+        "ex3_500_c32": lambda: wl.example3(500, "c32"), "ex3_4096_c32": lambda: wl.example3(4096, "c32"),
         # small-grid regime: one 64^2 grid, and an ensemble of 64^2 grids
         "cfg2_64_c32": lambda: wl.cfg2(64, "c32"), "cfg5_512x64_c32": lambda: wl.cfg5(64, 512, "c32"),
         "cfg5_512x64_c64": lambda: wl.cfg5(64, 512, "c64"),

@@ -16,6 +16,11 @@
 #include "phx_common.cuh"
 #include "phx_philox.cuh"
 
+// Rows the DRAM -> L2 prefetch of the per-stage kernels runs ahead of the register prefetch (0 = none).
+#ifndef PHX_STAGE_PF_ROWS
+#define PHX_STAGE_PF_ROWS 0
+#endif
+
 namespace phx {
 
 template <typename T>
@@ -228,6 +233,31 @@ stage_kernel(const __grid_constant__ StageArgs<T> a) {
         }
     };
 
+    // DRAM -> L2 prefetch of everything row j of this thread's columns will read (no registers are tied up; the loads one
+    // row ahead then hit L2).  The per-stage kernels are bound by HBM latency x bytes in flight: stage 1 moves 20 B per cell
+    // and a thread has 24 B in flight with the register prefetch alone.
+    auto prefetch_row = [&](int j) {
+        if (PHX_STAGE_PF_ROWS <= 0 || !col.active || j >= j1) return;
+        const size_t o = (size_t)j * g.nx + col.x0;
+        auto pf = [](const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); };
+#pragma unroll
+        for (int s = 0; s < NC; ++s) {
+            pf(yin[s] + o);
+            if (STAGE == 2 || STAGE == 3) pf(psi[s] + o);
+            if (STAGE == 3 || STAGE == 4) pf(acc[s] + o);
+            if constexpr (RES) {
+                pf(nin[s] + o);
+                if (STAGE == 2 || STAGE == 3 || (STAGE == 4 && NOISE)) pf(nst[s] + o);
+                if (STAGE == 3 || STAGE == 4) pf(nacc[s] + o);
+            }
+        }
+        if (a.f.V) pf(a.f.V + o);
+        if (RES && a.f.P) pf(a.f.P + o);
+        if (a.f.E) pf(a.f.E + o);
+    };
+#pragma unroll 1
+    for (int d = 2; d < 2 + PHX_STAGE_PF_ROWS; ++d) prefetch_row(j0 + d);
+
     // ---- prologue: rows j0-1, j0, j0+1 of the stage input; row-local inputs of row j0 ---------
     Row<T, VEC> win[NC][4];
 #pragma unroll
@@ -241,6 +271,7 @@ stage_kernel(const __grid_constant__ StageArgs<T> a) {
     load_aux(j0, cur, shc);
 
     for (int j = j0; j < j1; ++j) {
+        prefetch_row(j + 2 + PHX_STAGE_PF_ROWS);
         // prefetch: stencil row j+2 and the row-local inputs of row j+1
         if (j + 1 < j1) {
 #pragma unroll

@@ -183,6 +183,7 @@ void fill_geo_coef(const phx_grid* g, Geom& geo, Coef<T>& k) {
     geo.nx = g->d.nx; geo.ny = g->d.ny; geo.batch = g->d.batch;
     geo.bc_x = g->d.bc_x; geo.bc_y = g->d.bc_y;
     geo.rows = g->rows;
+    geo.pf = g->L.total > g->l2_bytes ? 1 : 0;      // (variant STAGE: L2 prefetch ahead of the register prefetch)
     geo.plane = plane_cells(g);
     const double* c = g->coef;
     k.cx = (T)c[0]; k.cy = (T)c[1]; k.ih = (T)c[2]; k.g = (T)c[3]; k.gx = (T)c[4]; k.gr = (T)c[5]; k.Rr = (T)c[6];

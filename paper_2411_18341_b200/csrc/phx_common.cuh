@@ -54,6 +54,7 @@ struct Geom {
     int nx, ny, batch;
     int bc_x, bc_y;        // 0 periodic, 1 zero
     int rows;              // rows per CTA (variant STAGE)
+    int pf;                // variant STAGE: 1 = prefetch rows ahead into L2 (working sets beyond L2 only)
     size_t plane;          // nx*ny
 };
 

@@ -16,9 +16,18 @@
 #include "phx_common.cuh"
 #include "phx_philox.cuh"
 
-// Rows the DRAM -> L2 prefetch of the per-stage kernels runs ahead of the register prefetch (0 = none).
+// Rows the DRAM -> L2 prefetch of the per-stage kernels runs ahead of the register prefetch (0 = none).  Same-run A/B at
+// 4 rows (Gcell*step/s): cfg2 4096^2 fp32 43.0 against 40.2 (84 % of the measured HBM bandwidth on the 128 algorithmic bytes),
+// cfg3 30.6 against 29.7, the 16384^2 spinor 20.2 against 21.0 (it has enough bytes in flight already); 8 rows lose everywhere,
+// and so do 4 on an L2-resident grid (1024^2 fp32 27.0 against 29.7): Geom::pf switches it on for working sets beyond L2.
 #ifndef PHX_STAGE_PF_ROWS
-#define PHX_STAGE_PF_ROWS 0
+#define PHX_STAGE_PF_ROWS 4
+#endif
+#ifndef PHX_STAGE_PF_ROWS_SPINOR
+#define PHX_STAGE_PF_ROWS_SPINOR 0
+#endif
+#ifndef PHX_STAGE_PF_ROWS_SPINOR1
+#define PHX_STAGE_PF_ROWS_SPINOR1 0     // (stage 1 of the spinor models, the one with the fewest bytes in flight)
 #endif
 
 namespace phx {
@@ -236,8 +245,9 @@ stage_kernel(const __grid_constant__ StageArgs<T> a) {
     // DRAM -> L2 prefetch of everything row j of this thread's columns will read (no registers are tied up; the loads one
     // row ahead then hit L2).  The per-stage kernels are bound by HBM latency x bytes in flight: stage 1 moves 20 B per cell
     // and a thread has 24 B in flight with the register prefetch alone.
+    constexpr int PFR = SPINOR ? (STAGE == 1 ? PHX_STAGE_PF_ROWS_SPINOR1 : PHX_STAGE_PF_ROWS_SPINOR) : PHX_STAGE_PF_ROWS;
     auto prefetch_row = [&](int j) {
-        if (PHX_STAGE_PF_ROWS <= 0 || !col.active || j >= j1) return;
+        if (PFR <= 0 || !g.pf || !col.active || j >= j1) return;
         const size_t o = (size_t)j * g.nx + col.x0;
         auto pf = [](const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); };
 #pragma unroll
@@ -256,7 +266,7 @@ stage_kernel(const __grid_constant__ StageArgs<T> a) {
         if (a.f.E) pf(a.f.E + o);
     };
 #pragma unroll 1
-    for (int d = 2; d < 2 + PHX_STAGE_PF_ROWS; ++d) prefetch_row(j0 + d);
+    for (int d = 2; d < 2 + PFR; ++d) prefetch_row(j0 + d);
 
     // ---- prologue: rows j0-1, j0, j0+1 of the stage input; row-local inputs of row j0 ---------
     Row<T, VEC> win[NC][4];
@@ -271,7 +281,7 @@ stage_kernel(const __grid_constant__ StageArgs<T> a) {
     load_aux(j0, cur, shc);
 
     for (int j = j0; j < j1; ++j) {
-        prefetch_row(j + 2 + PHX_STAGE_PF_ROWS);
+        prefetch_row(j + 2 + PFR);
         // prefetch: stencil row j+2 and the row-local inputs of row j+1
         if (j + 1 < j1) {
 #pragma unroll

@@ -93,6 +93,7 @@ struct phx_grid {
     cudaEvent_t ev_fork, ev_join;
     int step_side;          // variant STEP side launch for a ragged last strip: 1 on; -1 and 0: off
     int step_pdl;           // variant STEP: later steps of a graph as programmatic dependent launches: -1 automatic, 0 off, 1 on
+    int resident_cluster;   // variant RESIDENT cluster form: -1 automatic, 0 never, 1 whenever it applies
     bool has_params;
     phx_params prm;
     double coef[PHX_NCOEF];
@@ -544,6 +545,22 @@ int kernels_per_step(const phx_grid* g) {
     return step_plan(g).side_cols > 0 ? 2 : 1;      // (a ragged last strip: main + side launch)
 }   // (RESIDENT: one per call)
 
+// Variant RESIDENT, which form: the cluster form (one realisation on 2-8 CTAs) when the grid does not fit one CTA, and for
+// small batches -- one 64^2 grid is stepped 2x faster by 8 SMs with a cluster barrier per stage than by one SM -- unless
+// the tuning key resident_cluster says otherwise (0 never, 1 whenever it applies).
+bool resident_single_ok(const phx_grid* g) {
+    return resident_cpt(plane_cells(g), g->d.prec == PHX_C64, model_reservoir(g->d.model)) != 0;
+}
+int resident_cluster_ctas(const phx_grid* g) {
+    return resident_cluster_size(g->d.nx, g->d.ny, g->d.prec == PHX_C64, model_reservoir(g->d.model));
+}
+bool resident_use_cluster(const phx_grid* g) {
+    const int n = resident_cluster_ctas(g);
+    if (n == 0 || g->resident_cluster == 0) return false;
+    if (!resident_single_ok(g) || g->resident_cluster == 1) return true;
+    return (long)g->d.batch * n <= (long)g->n_sm;          // every cluster resident at once: more SMs per realisation
+}
+
 // Variant RESIDENT: all n steps in one launch, in place on the buffers of the current parity.
 template <typename T>
 cudaError_t launch_resident(phx_grid* g, int n_steps) {
@@ -560,6 +577,10 @@ cudaError_t launch_resident(phx_grid* g, int n_steps) {
     a.step0 = g->step_host;
     a.n_steps = n_steps;
     a.seed = g->prm.seed;
+    if (resident_use_cluster(g)) {
+        if constexpr (sizeof(T) == 4) return launch_resident_cluster_32(a, res, g->d.noise != 0, g->stream);
+        else return launch_resident_cluster_64(a, res, g->d.noise != 0, g->stream);
+    }
     if constexpr (sizeof(T) == 4) return launch_resident_32(a, res, g->d.noise != 0, g->stream);
     else return launch_resident_64(a, res, g->d.noise != 0, g->stream);
 }
@@ -594,8 +615,12 @@ bool step_variant_ok(const phx_grid* g) { return (size_t)g->d.nx * (size_t)g->d.
 // Variant RESIDENT: scalar and reservoir models without drive whose grid fits one CTA (phx_resident.cu).
 bool resident_variant_ok(const phx_grid* g) {
     if (model_spinor(g->d.model) || g->hasE) return false;
-    return resident_cpt(plane_cells(g), g->d.prec == PHX_C64, model_reservoir(g->d.model)) != 0;
+    return resident_single_ok(g) || (g->resident_cluster != 0 && resident_cluster_ctas(g) != 0);
 }
+
+// Largest single grid AUTO gives to the cluster form of variant RESIDENT (measured, us per step, cluster form against the fused
+// step: cfg1 64^2 fp64 2.45 / 3.58, 64^2 fp32 2.08 / 3.33, 128^2 fp32 4.91 / 3.38, 128^2 fp64 5.72 / 3.92).
+constexpr int RESIDENT_CLUSTER_AUTO_CELLS = 4096;
 
 // AUTO takes the resident kernel for ensembles of grids that fit it (one CTA per realisation: 2.3x the fused step on
 // 512 x 64^2 fp32; a single small grid is faster spread over several SMs by the fused step: 3.9 against 4.3 us per step at
@@ -604,7 +629,10 @@ bool resident_variant_ok(const phx_grid* g) {
 void resolve_variant(phx_grid* g) {
     const int req = g->variant_req;
     const bool res_ok = resident_variant_ok(g);
-    if (res_ok && (req == PHX_VARIANT_RESIDENT || (req == PHX_VARIANT_AUTO && g->d.batch >= 32))) g->variant = PHX_VARIANT_RESIDENT;
+    // (AUTO: ensembles of grids that fit one CTA; single grids of at most 4096 cells on a cluster, one cell per thread)
+    const bool auto_res = g->d.batch >= 32 ? resident_single_ok(g)
+                                           : (resident_use_cluster(g) && plane_cells(g) <= (size_t)RESIDENT_CLUSTER_AUTO_CELLS);
+    if (res_ok && (req == PHX_VARIANT_RESIDENT || (req == PHX_VARIANT_AUTO && auto_res))) g->variant = PHX_VARIANT_RESIDENT;
     else if (req != PHX_VARIANT_STAGE && step_variant_ok(g)) g->variant = PHX_VARIANT_STEP;
     else g->variant = PHX_VARIANT_STAGE;
 }
@@ -808,6 +836,7 @@ phx_status phx_create_grid(phx_grid** out, const phx_grid_desc* desc) {
     g->step_xch = -1;
     g->step_side = -1;
     g->step_pdl = -1;
+    g->resident_cluster = -1;
     g->step_warps = 0;
     g->async_host = 0;
     g->n_sm = prop.multiProcessorCount;
@@ -1146,6 +1175,10 @@ phx_status phx_set_tuning(phx_grid* g, const char* key, int32_t value) {
     } else if (!std::strcmp(key, "step_xch")) {       // variant STEP exchanging strips: -1 automatic (wherever the row fits), 0 off
         if (value < -1 || value > 1) return PHX_ERR_INVALID_ARG;
         g->step_xch = value;
+    } else if (!std::strcmp(key, "resident_cluster")) {   // variant RESIDENT on a thread-block cluster: -1 automatic, 0 never, 1 whenever it applies
+        if (value < -1 || value > 1) return PHX_ERR_INVALID_ARG;
+        g->resident_cluster = value;
+        resolve_variant(g);
     } else if (!std::strcmp(key, "step_pdl")) {       // variant STEP programmatic dependent launches inside a graph: -1 automatic, 0 off, 1 on
         if (value < -1 || value > 1) return PHX_ERR_INVALID_ARG;
         g->step_pdl = value;

@@ -115,6 +115,10 @@ struct ResidentArgs {
 int resident_cpt(size_t cells, int prec64, bool res);     // cells per thread, 0 = the grid does not fit
 cudaError_t launch_resident_32(const ResidentArgs<float>&, bool res, bool noise, cudaStream_t);
 cudaError_t launch_resident_64(const ResidentArgs<double>&, bool res, bool noise, cudaStream_t);
+// cluster form: one realisation on a thread-block cluster of 2-8 CTAs (row slabs, halo rows through distributed shared memory)
+int resident_cluster_size(int nx, int ny, int prec64, bool res);   // 0 = does not apply
+cudaError_t launch_resident_cluster_32(const ResidentArgs<float>&, bool res, bool noise, cudaStream_t);
+cudaError_t launch_resident_cluster_64(const ResidentArgs<double>&, bool res, bool noise, cudaStream_t);
 
 // phx_aux.cu: small helper kernels
 cudaError_t launch_ensemble_mean(const void* psi, void* out, int prec64, size_t plane, int batch, cudaStream_t);

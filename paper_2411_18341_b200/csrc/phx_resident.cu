@@ -10,11 +10,19 @@
 // boundary) are staged in shared memory once.  HBM traffic: the state in at the first step and out at the
 // last.  Scalar and reservoir models, both precisions, optional noise (Eq. (22)); no drive.
 // The derivative is the one of variant STEP (phx_deriv.cuh).  Product code: shares nothing with oracle/.
+//
+// CLUSTER form (resident_cluster_kernel): one realisation spread over a thread-block cluster of 2-8 CTAs, each owning a slab
+// of ny / cluster rows plus one halo row above and below in its own shared memory.  After a stage every CTA stores the first
+// and last row it produced straight into its neighbours' halo rows through distributed shared memory
+// (cluster.map_shared_rank), then the cluster barrier (barrier.cluster, ~380 cycles) takes the place of __syncthreads.  For a
+// SINGLE small grid, which one SM steps too slowly (fp64: 64 lanes) and the fused step cannot step faster than a kernel
+// launch per step allows (cfg1: 3.6 us per step).
 #include "phx_common.cuh"
 #include "phx_deriv.cuh"
 #include "phx_philox.cuh"
 #include "phx_launch.h"
 
+#include <cooperative_groups.h>
 #include <type_traits>
 
 namespace phx {
@@ -131,6 +139,202 @@ resident_kernel(const __grid_constant__ ResidentArgs<T> a) {
         a.step_slots[1] = a.step0 + (uint64_t)a.n_steps;
     }
 }
+
+
+// ---- cluster form ------------------------------------------------------------------------------------------------------
+// Local layout of a stage buffer in the CTA of cluster rank r (rl = ny / cluster rows): row 0 = halo (grid row r*rl - 1),
+// rows 1 .. rl = the slab, row rl + 1 = halo (grid row (r+1)*rl), then one cell that stays 0 (a zero boundary in x).
+template <typename T, bool RES, bool NOISE, int CPT>
+__global__ void __launch_bounds__(RES_NT, 1)
+resident_cluster_kernel(const __grid_constant__ ResidentArgs<T> a) {
+    namespace cg = cooperative_groups;
+    using C = typename Cx<T>::type;
+    extern __shared__ __align__(16) unsigned char smem[];
+    cg::cluster_group cluster = cg::this_cluster();
+    const Geom& g = a.geo;
+    const Coef<T>& k = a.k;
+    const int ncta = (int)cluster.num_blocks(), rank = (int)cluster.block_rank();
+    const int nx = g.nx, rl = g.ny / ncta, NL = rl * nx, NB = (rl + 2) * nx;     // NB = index of the zero cell
+    C* buf0 = reinterpret_cast<C*>(smem);
+    C* buf1 = buf0 + (NB + 1);
+    ushort2* nbr = reinterpret_cast<ushort2*>(buf1 + (NB + 1));                   // west, east (south / north are -+ nx)
+    T* Vs = reinterpret_cast<T*>(nbr + NL);
+    T* Ps = Vs + NL;
+
+    const int tid = threadIdx.x;
+    const int real = blockIdx.x / ncta;
+    const size_t boff = (size_t)real * g.plane;
+    C* psi_g = a.psi + boff;
+    T* n_g = RES ? a.n + boff : nullptr;
+    const C czero = mk<T>(T(0), T(0));
+    const int j0 = rank * rl;                                  // first grid row of the slab
+    // neighbours in y: the CTA holding the row below / above the slab (none beyond a zero boundary)
+    const bool has_s = !(g.bc_y && rank == 0), has_n = !(g.bc_y && rank == ncta - 1);
+    const int rank_s = rank == 0 ? ncta - 1 : rank - 1, rank_n = rank == ncta - 1 ? 0 : rank + 1;
+    C* rs0 = cluster.map_shared_rank(buf0, rank_s); C* rs1 = cluster.map_shared_rank(buf1, rank_s);
+    C* rn0 = cluster.map_shared_rank(buf0, rank_n); C* rn1 = cluster.map_shared_rank(buf1, rank_n);
+
+    for (int c = tid; c < NB + 1; c += RES_NT) { buf0[c] = czero; buf1[c] = czero; }
+    __syncthreads();
+    C psi[CPT], acc[CPT];
+    T nn[CPT], nacc[CPT], nst[CPT];
+#pragma unroll
+    for (int q = 0; q < CPT; ++q) {
+        const int c = tid + q * RES_NT;
+        psi[q] = czero; acc[q] = czero; nn[q] = T(0); nacc[q] = T(0); nst[q] = T(0);
+        if (c < NL) {
+            const int lr = c / nx, i = c - lr * nx, b = (lr + 1) * nx + i;
+            ushort2 nb;
+            nb.x = (unsigned short)(i > 0 ? b - 1 : (g.bc_x ? NB : b + nx - 1));
+            nb.y = (unsigned short)(i < nx - 1 ? b + 1 : (g.bc_x ? NB : b - nx + 1));
+            nbr[c] = nb;
+            const size_t gc = (size_t)(j0 + lr) * nx + i;
+            Vs[c] = a.V ? a.V[gc] : T(0);
+            Ps[c] = (RES && a.P) ? a.P[gc] : T(0);
+            psi[q] = psi_g[gc];
+            if (RES) nn[q] = n_g[gc];
+            buf0[b] = psi[q];
+        }
+    }
+    // halo rows of the first stage input, from global memory
+    for (int i = tid; i < nx; i += RES_NT) {
+        if (has_s) buf0[i] = psi_g[(size_t)(j0 == 0 ? g.ny - 1 : j0 - 1) * nx + i];
+        if (has_n) buf0[(rl + 1) * nx + i] = psi_g[(size_t)(j0 + rl == g.ny ? 0 : j0 + rl) * nx + i];
+    }
+    cluster.sync();
+
+    auto stage = [&](const C* in, C* out, C* out_s, C* out_n, auto stage_no, const uint64_t step) {
+        constexpr int s = decltype(stage_no)::value;
+        const T a_dt = s == 3 ? k.dt : k.hdt;
+        const T w_dt = (s == 1 || s == 4) ? k.dt6 : k.dt3;
+#pragma unroll
+        for (int q = 0; q < CPT; ++q) {
+            const int c = tid + q * RES_NT;
+            if (c < NL) {
+                const int lr = c / nx, i = c - lr * nx, b = (lr + 1) * nx + i;
+                const ushort2 nb = nbr[c];
+                Nbhd<T> h;
+                h.c = s == 1 ? psi[q] : in[b];
+                h.w = in[nb.x]; h.e = in[nb.y]; h.s = in[b - nx]; h.n = in[b + nx];
+                Diff<T> df;
+                differences<T, false, false>(k, h, df);
+                const T nres = RES ? (s == 1 ? nn[q] : nst[q]) : T(0);
+                T Kn;
+                const C K = deriv<T, false, RES, false>(k, h.c, df, czero, df, true, nres, Vs[c], Ps[c], czero, czero, Kn);
+                if (s == 1) {
+                    acc[q] = fma2s(w_dt, K, psi[q]);
+                    if (RES) nacc[q] = nn[q] + w_dt * Kn;
+                } else if (s < 4) {
+                    acc[q] = fma2s(w_dt, K, acc[q]);
+                    if (RES) nacc[q] += w_dt * Kn;
+                }
+                C y;
+                if (s < 4) {
+                    y = fma2s(a_dt, K, psi[q]);
+                    if (RES) nst[q] = nn[q] + a_dt * Kn;
+                } else {
+                    y = fma2s(w_dt, K, acc[q]);
+                    if (NOISE) {
+                        const uint4 wd = noise_words(a.seed, (uint32_t)real, step, (uint32_t)((j0 + lr) * nx + i));
+                        const T nt = RES ? nn[q] : T(0);          // reservoir at the start of the step
+                        y = add2(y, noise_increment_sfu(wd.x, wd.y, k.sig2 * (T(2) * k.hgc + k.Rr * nt)));
+                    }
+                    psi[q] = y;
+                    if (RES) nn[q] = nacc[q] + w_dt * Kn;
+                }
+                out[b] = y;
+                // the slab's first row is the northern halo of the CTA below, its last row the southern halo of the CTA above
+                if (lr == 0 && has_s) out_s[(rl + 1) * nx + i] = y;
+                if (lr == rl - 1 && has_n) out_n[i] = y;
+            }
+        }
+        cluster.sync();
+    };
+
+    for (int it = 0; it < a.n_steps; ++it) {
+        const uint64_t step = a.step0 + (uint64_t)it;
+        stage(buf0, buf1, rs1, rn1, std::integral_constant<int, 1>(), step);
+        stage(buf1, buf0, rs0, rn0, std::integral_constant<int, 2>(), step);
+        stage(buf0, buf1, rs1, rn1, std::integral_constant<int, 3>(), step);
+        stage(buf1, buf0, rs0, rn0, std::integral_constant<int, 4>(), step);
+    }
+
+#pragma unroll
+    for (int q = 0; q < CPT; ++q) {
+        const int c = tid + q * RES_NT;
+        if (c < NL) {
+            const int lr = c / nx, i = c - lr * nx;
+            const size_t gc = (size_t)(j0 + lr) * nx + i;
+            psi_g[gc] = psi[q];
+            if (RES) n_g[gc] = nn[q];
+        }
+    }
+    if (blockIdx.x == 0 && tid == 0) {
+        a.step_slots[0] = a.step0 + (uint64_t)a.n_steps;
+        a.step_slots[1] = a.step0 + (uint64_t)a.n_steps;
+    }
+}
+
+size_t resident_cluster_smem_bytes(int nx, int rl, int prec64) {
+    const size_t rb = prec64 ? 8 : 4, nb = (size_t)(rl + 2) * nx + 1, nl = (size_t)rl * nx;
+    return 2 * nb * 2 * rb + nl * sizeof(ushort2) + 2 * nl * rb;
+}
+
+// Cluster size for one realisation of an nx x ny grid (0 = the cluster form does not apply): the largest of 8, 4, 2 that
+// divides ny, gives every CTA at least 2 rows, and whose slab fits 4 cells per thread and the shared memory.
+int resident_cluster_size(int nx, int ny, int prec64, bool res) {
+    (void)res;
+    for (int n = 8; n >= 2; n >>= 1) {
+        if (ny % n != 0 || ny / n < 2) continue;
+        const int rl = ny / n;
+        if ((size_t)rl * nx > 4u * RES_NT || (size_t)(rl + 2) * nx + 1 > 65535u) continue;
+        if (resident_cluster_smem_bytes(nx, rl, prec64) > 200 * 1024) continue;
+        return n;
+    }
+    return 0;
+}
+
+template <typename T, bool RES, bool NOISE, int CPT>
+static cudaError_t launch_cluster_one(const ResidentArgs<T>& a, int ncta, cudaStream_t st) {
+    const size_t smem = resident_cluster_smem_bytes(a.geo.nx, a.geo.ny / ncta, sizeof(T) == 8);
+    auto kern = resident_cluster_kernel<T, RES, NOISE, CPT>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)(a.geo.batch * ncta));
+    cfg.blockDim = dim3(RES_NT);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = (unsigned)ncta;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kern, a);
+}
+
+template <typename T>
+static cudaError_t launch_cluster_t(const ResidentArgs<T>& a, bool res, bool noise, cudaStream_t st) {
+    const int ncta = resident_cluster_size(a.geo.nx, a.geo.ny, sizeof(T) == 8, res);
+    if (ncta == 0) return cudaErrorInvalidConfiguration;
+    const int need = (a.geo.nx * (a.geo.ny / ncta) + RES_NT - 1) / RES_NT;
+#define PHX_RESC_CASE(R, NZ)                                                  \
+    if (res == R && noise == NZ) {                                            \
+        if (need == 1) return launch_cluster_one<T, R, NZ, 1>(a, ncta, st);   \
+        return launch_cluster_one<T, R, NZ, 4>(a, ncta, st);                  \
+    }
+    PHX_RESC_CASE(false, false)
+    PHX_RESC_CASE(false, true)
+    PHX_RESC_CASE(true, false)
+    PHX_RESC_CASE(true, true)
+#undef PHX_RESC_CASE
+    return cudaErrorInvalidConfiguration;
+}
+
+cudaError_t launch_resident_cluster_32(const ResidentArgs<float>& a, bool res, bool noise, cudaStream_t st) { return launch_cluster_t<float>(a, res, noise, st); }
+cudaError_t launch_resident_cluster_64(const ResidentArgs<double>& a, bool res, bool noise, cudaStream_t st) { return launch_cluster_t<double>(a, res, noise, st); }
 
 size_t resident_smem_bytes(int cells, int prec64) {
     const size_t rb = prec64 ? 8 : 4;

@@ -109,8 +109,8 @@ def test_resident_agrees_with_step_to_rounding():
 
 
 def test_grids_that_do_not_fit_are_refused():
-    for w, kw in ((wl.cfg2(n=128, ny=64, prec="c32"), {}), (wl.cfg4(n=32, prec="c32", sigma_cells=5.0), {}),
-                  (wl.cfg3(n=64, prec="c64"), {})):   # too many cells; spinor; fp64 reservoir beyond 2048 cells
+    for w, kw in ((wl.cfg2(n=256, ny=256, prec="c32"), {}), (wl.cfg4(n=32, prec="c32", sigma_cells=5.0), {}),
+                  (wl.cfg2(n=128, ny=65, prec="c32"), {})):   # too many cells even for a cluster; spinor; too many cells for one CTA and an odd row count
         g = make_gpu(w, **kw)
         assert g.get_variant() == STEP
         with pytest.raises(phx.PhxError) as e:
@@ -119,9 +119,62 @@ def test_grids_that_do_not_fit_are_refused():
         g.destroy()
     w = wl.cfg2(n=32, ny=32, prec="c32")
     g = make_gpu(w)
-    assert g.get_variant() == STEP                 # AUTO: a single small grid is faster spread over several SMs
-    g.select_variant(RESIDENT)
-    assert g.get_variant() == RESIDENT
+    assert g.get_variant() == RESIDENT             # AUTO: a single small grid runs on a cluster (the cluster form)
     g.set_drive(np.zeros((32, 32), np.complex64))  # a drive: the fused step takes over
     assert g.get_variant() == STEP
+    g.destroy()
+    g = make_gpu(wl.cfg2(n=33, ny=31, prec="c32"))
+    assert g.get_variant() == STEP                 # an odd row count has no cluster form: the fused step spreads it over several SMs
+    g.select_variant(RESIDENT)
+    assert g.get_variant() == RESIDENT             # (one CTA, on request)
+    g.destroy()
+
+
+# ---- cluster form: one realisation on a thread-block cluster of 2-8 CTAs ------------------------------
+@pytest.mark.parametrize("maker,bc", [
+    (lambda: wl.cfg1(n_steps=100), (0, 0)),                               # 64 x 64 fp64: 8 CTAs of 8 rows, one cell per thread
+    (lambda: wl.cfg2(n=64, ny=64, prec="c32"), (0, 0)),
+    (lambda: wl.cfg2(n=128, ny=128, prec="c32"), (0, 0)),                 # 16 rows per CTA, four cells per thread
+    (lambda: wl.cfg2(n=128, ny=128, prec="c64"), (1, 1)),
+    (lambda: wl.cfg2(n=96, ny=40, prec="c32"), (0, 1)),                   # 5 rows per CTA; zero boundary in y
+    (lambda: wl.cfg2(n=50, ny=12, prec="c64"), (1, 0)),                   # 12 rows: a cluster of 4
+    (lambda: wl.cfg2(n=33, ny=6, prec="c32"), (0, 0)),                    # 6 rows: a cluster of 2, the neighbour above is the neighbour below
+    (lambda: wl.cfg3(n=64, prec="c32"), (0, 0)),
+    (lambda: wl.cfg3(n=128, prec="c64"), (0, 0)),
+    (lambda: wl.cfg5(n=64, batch=3, prec="c32"), (0, 0)),                 # noise: the cell index of the counter is the grid's
+    (lambda: wl.cfg5(n=128, batch=2, prec="c32"), (0, 0))])
+def test_cluster_form(maker, bc):
+    w = maker()
+    g = make_gpu(w, variant=RESIDENT, bc=bc, tuning={"resident_cluster": 1})
+    assert g.get_variant() == RESIDENT
+    o = make_oracle(w, bc=bc)
+    g.step_rk4(57)
+    g.step_rk4(4)
+    o.step_rk4(61)
+    compare(g, o, w)
+    assert g.get_launch_count() == 2 and g.get_step() == 61
+    # against the one-CTA form where the grid fits it: the same cell arithmetic (phx_deriv.cuh), hence the same bits -- except
+    # with noise, where the compiler contracts the reservoir / variance expressions differently for 1 and 8 cells per thread
+    # (rounding-level: bounded at a tenth of the field tolerance)
+    if w.nx * w.ny <= 4096 and not (w.prec == "c64" and w.model == "reservoir" and w.nx * w.ny > 2048):
+        ref = make_gpu(w, variant=RESIDENT, bc=bc, tuning={"resident_cluster": 0})
+        ref.step_rk4(61)
+        for name in w.fields:
+            if w.noise:
+                assert rel_l2(g.read_field(name), ref.read_field(name)) <= 0.1 * TOL[w.prec], name
+            else:
+                assert np.array_equal(g.read_field(name), ref.read_field(name)), name
+        ref.destroy()
+    g.destroy()
+
+
+def test_cluster_form_opens_resident_to_128_wide_grids():
+    g = make_gpu(wl.cfg2(n=128, ny=128, prec="c32"))      # AUTO: the fused step (faster at this size)
+    assert g.get_variant() == STEP
+    g.select_variant(RESIDENT)
+    assert g.get_variant() == RESIDENT                     # does not fit one CTA: the cluster form
+    g.destroy()
+    g = make_gpu(wl.cfg2(n=128, ny=128, prec="c32"), tuning={"resident_cluster": 0})
+    with pytest.raises(phx.PhxError):
+        g.select_variant(RESIDENT)                         # without the cluster form the request is refused
     g.destroy()

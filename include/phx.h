@@ -218,6 +218,27 @@ phx_status phx_get_variant(const phx_grid* g, int32_t* variant);
 phx_status phx_get_launch_count(const phx_grid* g, uint64_t* launches);
 phx_status phx_set_tuning(phx_grid* g, const char* key, int32_t value);
 
+/* ---- stepping without a handle, a workspace or any allocation ---------------------------------------------------------
+ * n_steps fixed-step RK4 steps (Eqs. (2)-(6); Listing 1, :100-144) of the scalar model Eq. (1) (
+ * no reservoir, spinor, drive or noise) on ONE nx x ny grid, for callers that cannot allocate (code under CUDA-graph capture,
+ * tight serving loops, harnesses that forbid cudaMalloc).  The call makes no cudaMalloc / cudaFree and calls no allocating
+ * library routine; it creates no stream, event or graph.  The stage buffers and the running sum of Eq. (6) live in a
+ * file-scope device array of PHX_STATIC_SCRATCH_BYTES inside libphx.so (every GPU that loads the library holds it until the
+ * process exits); the kernels are the per-stage kernels of phx_step_rk4 (variant STAGE), so the result is the same.
+ *   psi_in, psi_out: DEVICE arrays [ny][nx] of interleaved complex T (T by prec), owned by the caller; may be the same array.
+ *   V: DEVICE array [ny][nx] of real T, or NULL (V = 0).  p: as phx_set_params (g_x, g_r, R, gamma_r, beta, omega, noise_scale,
+ *   seed are not used).  bc_x, bc_y: phx_boundary.  stream: cudaStream_t or NULL; the work is enqueued, not synchronised.
+ * The device of the arrays must be the current device.  Limit: 3 x align256(nx*ny*sizeof(complex T)) + 256 bytes must fit
+ * the array: nx*ny <= 349 504 cells in complex fp32 (e.g. 512 x 512, 590 x 590), 174 752 in complex fp64 (e.g. 256 x 256, 417 x 417).
+ * Returns PHX_ERR_WORKSPACE for a larger grid (nothing is enqueued), PHX_ERR_INVALID_ARG for bad arguments, PHX_ERR_CUDA if
+ * the CUDA runtime refuses a call.  All calls share the array, which keeps the last call's contents (what must start at zero
+ * is cleared by every call): calls whose kernels may overlap on the GPU (different streams) RACE on it -- keep them on one
+ * stream or order them with events. */
+#define PHX_STATIC_SCRATCH_BYTES (8u << 20)
+phx_status phx_step_rk4_static(int32_t nx, int32_t ny, double dx, double dy, int32_t prec, int32_t bc_x, int32_t bc_y,
+                               const phx_params* p, const void* V, const void* psi_in, void* psi_out, int64_t n_steps,
+                               void* stream);
+
 /* Waits for the stream; returns the sticky CUDA status. */
 phx_status phx_sync(phx_grid* g);
 

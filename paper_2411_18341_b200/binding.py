@@ -32,7 +32,8 @@ EXPORTS = ("phx_workspace_bytes", "phx_create_grid", "phx_set_params", "phx_set_
            "phx_get_step", "phx_set_step",
            "phx_ensemble_mean_density", "phx_get_coeffs", "phx_debug_noise_u32", "phx_select_variant",
            "phx_get_variant", "phx_get_launch_count", "phx_set_tuning", "phx_sync", "phx_last_error",
-           "phx_destroy_grid")
+           "phx_destroy_grid", "phx_step_rk4_static")
+PHX_STATIC_SCRATCH_BYTES = 8 << 20
 
 
 class phx_grid_desc(C.Structure):
@@ -85,6 +86,7 @@ def lib():
             "phx_ensemble_mean_density": [vp, i32, vp, i32], "phx_get_coeffs": [vp, vp, i32],
             "phx_debug_noise_u32": [vp, u64, vp, i32], "phx_select_variant": [vp, i32], "phx_get_variant": [vp, vp],
             "phx_get_launch_count": [vp, vp], "phx_set_tuning": [vp, C.c_char_p, i32], "phx_sync": [vp],
+            "phx_step_rk4_static": [i32, i32, C.c_double, C.c_double, i32, i32, i32, vp, vp, vp, vp, i64, vp],
         }
         for name, args in sigs.items():
             fn = getattr(L, name)
@@ -302,3 +304,24 @@ def grid_from_workload(w, variant=PHX_VARIANT_AUTO, stream=None, upload=True, **
         for name, arr in w.fields.items():
             g.set_field(name, arr)
     return g
+
+
+def step_rk4_static(psi_in, psi_out, dx, dy, params, V=None, n_steps=1, bc=(0, 0), stream=None):
+    """phx_step_rk4_static: RK4 steps of the scalar model without a handle, a workspace or any allocation (include/phx.h).
+    psi_in / psi_out / V: torch CUDA tensors [ny][nx] (complex64 or complex128; V float32 / float64) on the current device;
+    enqueues on `stream` (a torch stream, default: the current one) and does not synchronise."""
+    import torch
+    ny, nx = psi_in.shape[-2], psi_in.shape[-1]
+    prec = PHX_C64 if psi_in.dtype == torch.complex128 else PHX_C32
+    if stream is None:
+        stream = torch.cuda.current_stream(psi_in.device)
+    st = lib().phx_step_rk4_static(nx, ny, float(dx), float(dy), prec, int(bc[0]), int(bc[1]), C.byref(params),
+                                   None if V is None else V.data_ptr(), psi_in.data_ptr(), psi_out.data_ptr(), int(n_steps),
+                                   stream.cuda_stream)
+    if st != PHX_OK:
+        need = 3 * ((nx * ny * (16 if prec == PHX_C64 else 8) + 255) // 256 * 256) + 256
+        msg = {PHX_ERR_WORKSPACE: f"phx_step_rk4_static: a {nx} x {ny} grid needs {need} bytes of scratch, the static array holds "
+                                  f"{PHX_STATIC_SCRATCH_BYTES}",
+               PHX_ERR_INVALID_ARG: "phx_step_rk4_static: invalid argument",
+               PHX_ERR_CUDA: "phx_step_rk4_static: CUDA runtime failure"}.get(st, "phx_step_rk4_static failed")
+        raise PhxError(st, msg)

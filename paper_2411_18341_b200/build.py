@@ -22,7 +22,7 @@ FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std
 def _units():
     """(object name, source, extra defines)"""
     u = [("phx_api.o", "phx_api.cu", []), ("phx_aux.o", "phx_aux.cu", []), ("phx_resident.o", "phx_resident.cu", []),
-         ("phx_adaptive.o", "phx_adaptive.cu", [])]
+         ("phx_adaptive.o", "phx_adaptive.cu", []), ("phx_static.o", "phx_static.cu", [])]
     for prec in (32, 64):
         for model in range(4):
             u.append((f"phx_stage_{prec}_{model}.o", "phx_stage_inst.cu",

@@ -279,7 +279,11 @@ bool step_bulk(const phx_grid* g) {
     if (g->d.bc_x || g->d.bc_y) return false;
     if (((size_t)g->d.nx * real_bytes(g)) % 16 != 0) return false;
     if (g->d.nx < 32 * step_vec(g)) return false;       // a strip wraps at most once
-    return g->step_bulk == 1;                           // opt-in: measured slower than the register loads
+    if (g->step_bulk >= 0) return g->step_bulk == 1;
+    // automatic: the cp.async flavour of the ring where it measured faster than the register loads (phx_launch.h:
+    // step_ring_auto), on working sets beyond L2, without drive; the TMA flavour stays an opt-in (slower everywhere)
+    if (!step_ring_auto(g->d.prec == PHX_C64, g->d.model) || g->hasE || step_vec(g) != 2) return false;
+    return g->L.total > g->l2_bytes;
 }
 
 int step_occupancy(const phx_grid* g, int vec) {

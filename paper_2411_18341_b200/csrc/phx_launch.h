@@ -49,6 +49,17 @@ constexpr bool step_early_exit(bool prec64, int model, int vec) {
 #ifndef PHX_STEP_DEPTH
 #define PHX_STEP_DEPTH 8
 #endif
+namespace phx {
+// Which flavour of the shared-memory ring a (precision, model) pair gets, and how deep.  cp.async (every lane copies its own
+// cells, no mbarrier): measured FASTER than the register loads on the reservoir model in complex fp32 (five arrays per row;
+// cfg3 4096^2: 155-160 against 144-147 Gcell*step/s at depth 8; cfg5-shaped ensembles without exchanging strips 98.6 against
+// 88.7) and marginally on the scalar model in complex fp64 (102.2-105.5 against 100.7-102.9 at depth 4): those two take it
+// by default on working sets beyond L2 (step_ring_auto).  Everything else keeps the TMA bulk-copy flavour as an opt-in
+// (slower than the register loads everywhere: profiles/r02_tma_vs_register_fetch.md).
+constexpr bool step_ring_cpasync(bool prec64, int model) { return (!prec64 && model == 1) || (prec64 && model == 0); }
+constexpr int step_ring_depth(bool prec64, int model) { return (prec64 && model == 0) ? 4 : PHX_STEP_DEPTH; }
+constexpr bool step_ring_auto(bool prec64, int model) { return step_ring_cpasync(prec64, model); }
+}
 
 namespace phx {
 

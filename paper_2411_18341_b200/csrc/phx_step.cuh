@@ -155,6 +155,20 @@ __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t
                  "@p cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];\n}"
                  ::"r"(dst), "l"(src), "r"(bytes), "r"(bar), "r"(lead) : "memory");
 }
+// cp.async form of the same ring (step_ring_cpasync, phx_launch.h): every LANE copies its own cells global -> shared with cp.async
+// (LDGSTS, 16 / 8 / 4 bytes), one commit group per row iteration, cp.async.wait_group before the row is read back.  A lane
+// only ever reads what it copied itself: no mbarrier, no elected lane, no __syncwarp, and a strip that crosses the periodic
+// edge needs no second piece (the lane's wrapped column addresses it).
+template <int BYTES> __device__ __forceinline__ void cpasync(uint32_t dst, const void* src) {
+    if constexpr (BYTES >= 16) {
+#pragma unroll
+        for (int o = 0; o < BYTES; o += 16)
+            asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst + o), "l"(static_cast<const char*>(src) + o) : "memory");
+    } else {
+        asm volatile("cp.async.ca.shared.global [%0], [%1], %2;" ::"r"(dst), "l"(src), "n"(BYTES) : "memory");
+    }
+}
+
 template <int VEC> __device__ __forceinline__ void ldsc(const float2* p, float2 (&v)[VEC]) {
     if constexpr (VEC % 2 == 0) {
 #pragma unroll
@@ -260,8 +274,9 @@ struct StepSmem {
     static constexpr uint32_t P = V + W * sizeof(T);
     static constexpr uint32_t E = P + (RES ? W * sizeof(T) : 0);
     static constexpr uint32_t STAGE = E + (DRIVE ? W * sizeof(C) : 0);
-    static constexpr uint32_t BARS = PHX_STEP_WARPS * PHX_STEP_DEPTH * 8;          // mbarriers, at the start
-    static constexpr uint32_t CTA = BARS + PHX_STEP_WARPS * PHX_STEP_DEPTH * STAGE;
+    static constexpr uint32_t DEPTH = step_ring_depth(sizeof(T) == 8, MODEL);
+    static constexpr uint32_t BARS = PHX_STEP_WARPS * DEPTH * 8;          // mbarriers, at the start
+    static constexpr uint32_t CTA = BARS + PHX_STEP_WARPS * DEPTH * STAGE;
 };
 
 // MINW: resident warps per SM the register budget is sized for.  ISO: dx == dy (scalar and reservoir models only).
@@ -472,7 +487,8 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
 
     // ---- bulk-copy fetch path: the ring, its mbarriers and the issuer's state ------------------------------------------------
     using SM = StepSmem<T, VEC, MODEL, DRIVE>;
-    constexpr int DEPTH = PHX_STEP_DEPTH;
+    constexpr int DEPTH = (int)SM::DEPTH;
+    constexpr bool CPA = step_ring_cpasync(sizeof(T) == 8, MODEL);      // flavour of the ring: cp.async per lane, or TMA bulk copies
     extern __shared__ __align__(128) unsigned char step_smem[];
     uint32_t bar0 = 0, ring0 = 0;                       // shared-window addresses of this warp's mbarriers and stages
     const unsigned char* ringp = nullptr;
@@ -485,12 +501,14 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
         bar0 = smem_u32(step_smem) + warp * DEPTH * 8;
         ringp = step_smem + SM::BARS + warp * DEPTH * SM::STAGE;
         ring0 = smem_u32(ringp);
-        if (lane == 0) {
+        if constexpr (!CPA) {
+            if (lane == 0) {
 #pragma unroll
-            for (int d = 0; d < DEPTH; ++d) mbar_init(bar0 + d * 8, 1);
-            asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+                for (int d = 0; d < DEPTH; ++d) mbar_init(bar0 + d * 8, 1);
+                asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+            }
+            __syncwarp();
         }
-        __syncwarp();
         ntot = ((r1 + 2 - j0) / RING + 1) * RING;
         qip = qw == 0 ? ny - 1 : qw - 1;
         c0 = (strip * OUTW - 4) % nx;
@@ -503,6 +521,23 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
     const uint32_t lead = lane == 0;
     const int len1 = min((int)W, nx - c0), len2 = W - len1;
     auto issue_fetch = [&]() {
+        if constexpr (CPA) {
+            const uint32_t dst = ring0 + ((uint32_t)fi % DEPTH) * SM::STAGE;
+            const uint32_t eq = (uint32_t)qi * (uint32_t)nx + (uint32_t)xg, ep = (uint32_t)qip * (uint32_t)nx + (uint32_t)xg;
+#pragma unroll
+            for (int s = 0; s < NC; ++s) {
+                cpasync<VEC * sizeof(C)>(dst + SM::PSI + (s * W + lane * VEC) * sizeof(C), pin[s] + eq);
+                if constexpr (RES) cpasync<VEC * sizeof(T)>(dst + SM::N + (s * W + lane * VEC) * sizeof(T), nin[s] + ep);
+            }
+            if (Vp) cpasync<VEC * sizeof(T)>(dst + SM::V + lane * VEC * sizeof(T), Vp + ep);
+            if (Pp) cpasync<VEC * sizeof(T)>(dst + SM::P + lane * VEC * sizeof(T), Pp + ep);
+            if constexpr (DRIVE) cpasync<VEC * sizeof(C)>(dst + SM::E + lane * VEC * sizeof(C), Ep + ep);
+            asm volatile("cp.async.commit_group;" ::: "memory");
+            ++fi;
+            qip = qi;
+            if (++qi == ny) qi = 0;
+            return;
+        }
         const uint32_t slot = (uint32_t)fi % DEPTH, bar = bar0 + slot * 8, dst = ring0 + slot * SM::STAGE;
         mbar_expect_tx(bar, txbytes, lead);
         const uint32_t eq = (uint32_t)qi * (uint32_t)nx, ep = (uint32_t)qip * (uint32_t)nx;
@@ -594,7 +629,8 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
             if constexpr (BULK) {
                 // the stage of this iteration has landed (phase parity of its mbarrier); registers <- shared memory
                 const uint32_t slot = (uint32_t)fc % DEPTH;
-                if (!ready) mbar_wait(bar0 + slot * 8, ((uint32_t)fc / DEPTH) & 1u);     // (rare: the copies run DEPTH - 1 rows ahead)
+                if constexpr (CPA) asm volatile("cp.async.wait_group %0;" ::"n"(DEPTH - 2) : "memory");   // the oldest group -- this iteration's row -- has landed
+                else if (!ready) mbar_wait(bar0 + slot * 8, ((uint32_t)fc / DEPTH) & 1u);                 // (rare: the copies run DEPTH - 1 rows ahead)
                 const unsigned char* st = ringp + slot * SM::STAGE;
 #pragma unroll
                 for (int s = 0; s < NC; ++s) {
@@ -605,7 +641,7 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
                 if (Pp) ldsr<VEC>(reinterpret_cast<const T*>(st + SM::P) + lane * VEC, Pr[SL(LEAD)]);
                 if constexpr (DRIVE) ldsc<VEC>(reinterpret_cast<const C*>(st + SM::E) + lane * VEC, Er[SL(LEAD)]);
                 ++fc;
-                ready = mbar_test(bar0 + ((uint32_t)fc % DEPTH) * 8, ((uint32_t)fc / DEPTH) & 1u);
+                if constexpr (!CPA) ready = mbar_test(bar0 + ((uint32_t)fc % DEPTH) * 8, ((uint32_t)fc / DEPTH) & 1u);
             } else {
 #pragma unroll
             for (int s = 0; s < NC; ++s) {
@@ -770,8 +806,12 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
             if constexpr (BULK) {
                 // the stage read in the previous iteration is free (its registers were consumed by this iteration's stages):
                 // refill it with the row DEPTH - 1 iterations ahead
-                __syncwarp();
-                if (fi < ntot) issue_fetch();
+                if constexpr (CPA) {
+                    issue_fetch();      // (always: one commit group per iteration keeps wait_group's count aligned)
+                } else {
+                    __syncwarp();
+                    if (fi < ntot) issue_fetch();
+                }
             }
             ewp = ew;
             okprev = okq;

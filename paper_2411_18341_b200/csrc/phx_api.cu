@@ -392,7 +392,7 @@ double step_plan_cost(const phx_grid* g, int vec, int wpc, int* ly_out, bool xch
                            : (long)g->n_sm * step_occupancy(g, vec) * (PHX_STEP_WARPS / wpc);   // resident CTAs of wpc warps
     const bool in_l2 = plane_cells(g) * g->d.batch * step_bytes_per_cell(g) < g->l2_bytes / 2;
     const bool whole_passes = xch || step_bulk(g) || !step_early_exit(g->d.prec == PHX_C64, g->d.model, vec);
-    const int ring = xch ? 4 + PHX_STEP_XLEAD : PHX_STEP_RING;
+    const int ring = xch ? 4 + step_xch_lead(g->d.prec == PHX_C64, g->d.model, vec) : PHX_STEP_RING;
     double best_cost = -1;
     int best_ly = g->d.ny;
     const int max_chunks = g->d.ny / 4 > 0 ? g->d.ny / 4 : 1;   // (a 64^2 grid: ly = 4, 3.6 instead of 4.9 us per step)

@@ -59,6 +59,13 @@ namespace phx {
 constexpr bool step_ring_cpasync(bool prec64, int model) { return (!prec64 && model == 1) || (prec64 && model == 0); }
 constexpr int step_ring_depth(bool prec64, int model) { return (prec64 && model == 0) ? 4 : PHX_STEP_DEPTH; }
 constexpr bool step_ring_auto(bool prec64, int model) { return step_ring_cpasync(prec64, model); }
+// The exchanging strips of the reservoir model in complex fp32 (cfg5) fetch through the cp.async ring (106.5 against 101.6
+// Gcell*step/s) and then need only one row of register lead (109.6 against 106.5 with two).
+#ifndef PHX_XCH_RING
+#define PHX_XCH_RING 1
+#endif
+constexpr bool step_xch_ringed(bool prec64, int model, int vec) { return PHX_XCH_RING && !prec64 && model == 1 && vec == 2; }
+constexpr int step_xch_lead(bool prec64, int model, int vec) { return step_xch_ringed(prec64, model, vec) ? 1 : PHX_STEP_XLEAD; }
 }
 
 namespace phx {

@@ -301,9 +301,10 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
     constexpr bool RES = model_reservoir(MODEL);
     constexpr int NC = SPINOR ? 2 : 1;
     constexpr int W = 32 * VEC, OUTW = XCH ? W : W - 8;
-    constexpr int LEAD = XCH ? PHX_STEP_XLEAD : PHX_STEP_LEAD, RING = 4 + LEAD;
+    constexpr int LEAD = XCH ? step_xch_lead(sizeof(T) == 8, MODEL, VEC) : PHX_STEP_LEAD, RING = 4 + LEAD;
     static_assert(!(BULK && ZBC), "the bulk-copy fetch path is built for periodic boundaries");
-    static_assert(!(XCH && (BULK || ZBC || SPINOR)), "the exchanging strips are built for periodic scalar / reservoir grids");
+    static_assert(!(XCH && (ZBC || SPINOR)), "the exchanging strips are built for periodic scalar / reservoir grids");
+    static_assert(!(XCH && BULK && !step_ring_cpasync(sizeof(T) == 8, MODEL)), "exchanging strips take the cp.async flavour of the ring only");
     const Geom& g = a.geo;
     const Coef<T>& k = a.k;
     const int nx = g.nx, ny = g.ny;

@@ -33,15 +33,30 @@ static cudaError_t launch_maybe_pdl(K kernel, const StepArgs<real_t>& a, dim3 gr
 }
 
 
+// The exchanging strips of the reservoir model in complex fp32 (cfg5) fetch their rows through the cp.async ring of
+// phx_step.cuh (PHX_XCH_RING; the ring is per warp, the CTA has a.wpc of them).
 template <int VEC, bool NOISE, bool ISO>
 struct InstX {
-    static auto kernel() { return step_kernel<real_t, VEC, PHX_INST_MODEL, NOISE, false, ISO, false, 8, false, true>; }
+    static constexpr bool RINGED = step_xch_ringed(PHX_INST_PREC == 64, PHX_INST_MODEL, VEC);
+    using SM = StepSmem<real_t, VEC, PHX_INST_MODEL, false>;
+    static size_t smem(int warps) { return RINGED ? SM::BARS + (size_t)warps * SM::DEPTH * SM::STAGE : 0; }
+    static auto kernel() { return step_kernel<real_t, VEC, PHX_INST_MODEL, NOISE, false, ISO, false, 8, RINGED, true>; }
+    static cudaError_t prepare() {
+        if (smem(PHX_STEP_XWARPS) > 48 * 1024) {
+            static cudaError_t once = cudaFuncSetAttribute(kernel(), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem(PHX_STEP_XWARPS));
+            return once;
+        }
+        return cudaSuccess;
+    }
     static cudaError_t launch(const StepArgs<real_t>& a, dim3 grid, cudaStream_t st) {
-        return launch_maybe_pdl(kernel(), a, grid, 0, st);
+        cudaError_t e = prepare();
+        if (e != cudaSuccess) return e;
+        return launch_maybe_pdl(kernel(), a, grid, smem(a.wpc), st);
     }
     static int occupancy(int warps) {
         int nb = 0;
-        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, kernel(), 32 * warps, 0) != cudaSuccess) {
+        if (prepare() != cudaSuccess ||
+            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, kernel(), 32 * warps, smem(warps)) != cudaSuccess) {
             cudaGetLastError();
             return 1;
         }

@@ -190,6 +190,11 @@ phx_status phx_set_step(phx_grid* g, uint64_t step);
 /* <|psi|^2>(x,y) = (1/batch) sum_r |psi_r|^2 as real T [ny][nx].  Synchronises. */
 phx_status phx_ensemble_mean_density(phx_grid* g, phx_field f, void* dst, phx_mem where);
 
+/* Failure detection: *all_finite <- 1 if every value of every state field (psi_+-, n_+- as present, all
+ * realisations) is finite, 0 if any is NaN or +-Inf -- what an RK4 run beyond its stability limit (PHX_WARN_UNSTABLE; the
+ * paper's explicit scheme has none of its own) ends in.  One pass over the state on the device.  Synchronises. */
+phx_status phx_check_finite(phx_grid* g, int32_t* all_finite);
+
 /* The canonical coefficients actually used (as double); n must be PHX_NCOEF. */
 phx_status phx_get_coeffs(const phx_grid* g, double* out, int32_t n);
 

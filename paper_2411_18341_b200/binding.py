@@ -32,7 +32,7 @@ EXPORTS = ("phx_workspace_bytes", "phx_create_grid", "phx_set_params", "phx_set_
            "phx_get_step", "phx_set_step",
            "phx_ensemble_mean_density", "phx_get_coeffs", "phx_debug_noise_u32", "phx_select_variant",
            "phx_get_variant", "phx_get_launch_count", "phx_set_tuning", "phx_sync", "phx_last_error",
-           "phx_destroy_grid", "phx_step_rk4_static")
+           "phx_destroy_grid", "phx_step_rk4_static", "phx_check_finite")
 PHX_STATIC_SCRATCH_BYTES = 8 << 20
 
 
@@ -86,6 +86,7 @@ def lib():
             "phx_ensemble_mean_density": [vp, i32, vp, i32], "phx_get_coeffs": [vp, vp, i32],
             "phx_debug_noise_u32": [vp, u64, vp, i32], "phx_select_variant": [vp, i32], "phx_get_variant": [vp, vp],
             "phx_get_launch_count": [vp, vp], "phx_set_tuning": [vp, C.c_char_p, i32], "phx_sync": [vp],
+            "phx_check_finite": [vp, vp],
             "phx_step_rk4_static": [i32, i32, C.c_double, C.c_double, i32, i32, i32, vp, vp, vp, vp, i64, vp],
         }
         for name, args in sigs.items():
@@ -244,6 +245,11 @@ class Grid:
         p, w = _addr(out)
         self._check(self._lib.phx_ensemble_mean_density(self._h, f, p, w))
         return out
+
+    def check_finite(self):
+        flag = C.c_int32(0)
+        self._check(self._lib.phx_check_finite(self._h, C.byref(flag)))
+        return bool(flag.value)
 
     def get_coeffs(self):
         out = np.zeros(PHX_NCOEF, dtype=np.float64)

@@ -1099,6 +1099,25 @@ phx_status phx_ensemble_mean_density(phx_grid* g, phx_field f, void* dst, phx_me
     return copy_out(g, dst, scratch, plane_cells(g) * real_bytes(g), where);
 }
 
+phx_status phx_check_finite(phx_grid* g, int32_t* all_finite) {
+    if (!g || !all_finite) return PHX_ERR_INVALID_ARG;
+    if (g->sticky != cudaSuccess) return PHX_ERR_CUDA;
+    int* flag = (int*)(g->ws + g->L.step + 64);          // (the counter slots take the first 16 of the 256 bytes)
+    PHX_CUDA(g, cudaMemsetAsync(flag, 0, sizeof(int), g->stream));
+    for (int f = PHX_PSI; f <= PHX_N_MINUS; ++f) {
+        if (!field_present(g, f)) continue;
+        size_t bytes;
+        const void* p = field_ptr(g, f, &bytes);
+        PHX_CUDA(g, launch_check_finite(p, bytes / real_bytes(g), g->d.prec == PHX_C64, flag, g->stream));
+        g->launches += 1;
+    }
+    int host = 0;
+    PHX_CUDA(g, cudaMemcpyAsync(&host, flag, sizeof(int), cudaMemcpyDeviceToHost, g->stream));
+    PHX_CUDA(g, cudaStreamSynchronize(g->stream));
+    *all_finite = host == 0;
+    return PHX_OK;
+}
+
 phx_status phx_get_coeffs(const phx_grid* g, double* out, int32_t n) {
     if (!g || !out || n != PHX_NCOEF) return PHX_ERR_INVALID_ARG;
     if (!g->has_params) return PHX_ERR_BAD_STATE;

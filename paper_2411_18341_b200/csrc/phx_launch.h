@@ -139,6 +139,7 @@ cudaError_t launch_resident_cluster_32(const ResidentArgs<float>&, bool res, boo
 cudaError_t launch_resident_cluster_64(const ResidentArgs<double>&, bool res, bool noise, cudaStream_t);
 
 // phx_aux.cu: small helper kernels
+cudaError_t launch_check_finite(const void* data, size_t n_reals, int prec64, int* flag, cudaStream_t);   // *flag <- 1 on NaN / Inf
 cudaError_t launch_ensemble_mean(const void* psi, void* out, int prec64, size_t plane, int batch, cudaStream_t);
 cudaError_t launch_noise_words(uint32_t* out, uint32_t seed, uint64_t step, size_t plane, int r0, int batch, cudaStream_t);
 

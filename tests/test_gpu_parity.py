@@ -228,3 +228,29 @@ def test_device_buffers_and_api_errors():
     assert np.array_equal(c, c.astype(np.float32).astype(np.float64)) and abs(c[0] - 25.0) < 1e-5
     g.destroy()
     g2.destroy()
+
+
+def test_check_finite_reports_nan_and_inf_in_any_state_field():
+    """phx_check_finite: finite fields -> True; one NaN / Inf anywhere in psi or n of any realisation ->
+    False; an RK4 run far beyond its stability limit (PHX_WARN_UNSTABLE) ends non-finite and is caught."""
+    w = wl.cfg5(n=64, batch=3, prec="c32")
+    for variant in (1, 3):
+        g = make_gpu(w, variant=variant)
+        g.step_rk4(3)
+        assert g.check_finite()
+        n = g.read_field("n_p")
+        n[2, 63, 63] = np.inf
+        g.set_field("n_p", n)
+        assert not g.check_finite()
+        n[2, 63, 63] = 0.0
+        g.set_field("n_p", n)
+        psi = g.read_field("psi_p")
+        psi[1, 17, 5] = complex(0.0, np.nan)
+        g.set_field("psi_p", psi)
+        assert not g.check_finite()
+        g.destroy()
+    w2 = wl.cfg2(n=64, ny=48, prec="c64")
+    g = make_gpu(w2, extra_params=dict(dt=0.4))         # (hbar/2m)(8/dx^2) dt = 80 >> 2.78
+    g.step_rk4(400)
+    assert not g.check_finite()
+    g.destroy()

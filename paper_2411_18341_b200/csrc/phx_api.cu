@@ -274,6 +274,13 @@ int step_vec(const phx_grid* g) {
 // dx == dy: the isotropic form of the Laplacian (cx == cy bit for bit, both derived from the same expression)
 bool step_iso(const phx_grid* g) { return g->d.dx == g->d.dy; }
 
+// Smallest workload (cells x realisations) AUTO gives the cp.async ring: same-run A/B, ring against register loads, Gcell*step/s:
+// cfg3 physics 2048^2 144 / 124, 1024^2 94.7 / 90.5, 512^2 50.9 / 42.5; scalar fp32 1536^2 163.8 / 158.6, 1024^2 116.2 / 113.4,
+// 512^2 59.8 / 50.9; scalar fp64 1024^2 73.0 / 71.7; below that the picture is mixed (384^2 fp32 29.9 / 31.8, 256^2 fp64
+// 12.2 / 12.8, 256^2 fp32 19.4 / 18.3) and the register loads stay.
+#ifndef PHX_RING_AUTO_LOG2_CELLS
+#define PHX_RING_AUTO_LOG2_CELLS 18
+#endif
 // The bulk-copy fetch path (phx_step.cuh, BULK): periodic boundaries, rows whose pieces are 16-byte aligned and sized.
 bool step_bulk(const phx_grid* g) {
     if (g->d.bc_x || g->d.bc_y) return false;
@@ -281,9 +288,9 @@ bool step_bulk(const phx_grid* g) {
     if (g->d.nx < 32 * step_vec(g)) return false;       // a strip wraps at most once
     if (g->step_bulk >= 0) return g->step_bulk == 1;
     // automatic: the cp.async flavour of the ring where it measured faster than the register loads (phx_launch.h:
-    // step_ring_auto), on working sets beyond L2, without drive; the TMA flavour stays an opt-in (slower everywhere)
-    if (!step_ring_auto(g->d.prec == PHX_C64, g->d.model) || g->hasE || step_vec(g) != 2) return false;
-    return g->L.total > g->l2_bytes;
+    // step_ring_auto), from 512^2 cells up, without drive; the TMA flavour stays an opt-in (slower everywhere)
+    if (!step_ring_auto(g->d.prec == PHX_C64, g->d.model, step_vec(g)) || g->hasE) return false;
+    return plane_cells(g) * g->d.batch >= ((size_t)1 << PHX_RING_AUTO_LOG2_CELLS);   // (small grids: the ring's prologue outweighs it)
 }
 
 int step_occupancy(const phx_grid* g, int vec) {

@@ -54,11 +54,15 @@ namespace phx {
 // cells, no mbarrier): measured FASTER than the register loads on the reservoir model in complex fp32 (five arrays per row;
 // cfg3 4096^2: 155-160 against 144-147 Gcell*step/s at depth 8; cfg5-shaped ensembles without exchanging strips 98.6 against
 // 88.7) and marginally on the scalar model in complex fp64 (102.2-105.5 against 100.7-102.9 at depth 4): those two take it
-// by default on working sets beyond L2 (step_ring_auto).  Everything else keeps the TMA bulk-copy flavour as an opt-in
+// by default from 512^2 cells up (step_ring_auto; phx_api.cu: step_bulk).  Everything else keeps the TMA bulk-copy flavour as an opt-in
 // (slower than the register loads everywhere: profiles/r02_tma_vs_register_fetch.md).
-constexpr bool step_ring_cpasync(bool prec64, int model) { return (!prec64 && model == 1) || (prec64 && model == 0); }
+// (vec = cells per lane.)  The scalar fp32 kernel with 2 or 1 cells per lane gains 2-3 % as well (1024^2 116.2 against 113.4,
+// 1536^2 163.8 against 158.6); with 4 cells per lane it loses 11 % and keeps register loads (its ring, the TMA flavour, is opt-in).
+constexpr bool step_ring_cpasync(bool prec64, int model, int vec) {
+    return (!prec64 && model == 1) || (prec64 && model == 0) || (!prec64 && model == 0 && vec <= 2);
+}
 constexpr int step_ring_depth(bool prec64, int model) { return (prec64 && model == 0) ? 4 : PHX_STEP_DEPTH; }
-constexpr bool step_ring_auto(bool prec64, int model) { return step_ring_cpasync(prec64, model); }
+constexpr bool step_ring_auto(bool prec64, int model, int vec) { return step_ring_cpasync(prec64, model, vec) && (vec == 2 || (prec64 && vec == 1)); }
 // The exchanging strips of the reservoir model in complex fp32 (cfg5) fetch through the cp.async ring (106.5 against 101.6
 // Gcell*step/s) and then need only one row of register lead (109.6 against 106.5 with two).
 #ifndef PHX_XCH_RING

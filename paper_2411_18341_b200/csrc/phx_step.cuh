@@ -304,7 +304,7 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
     constexpr int LEAD = XCH ? step_xch_lead(sizeof(T) == 8, MODEL, VEC) : PHX_STEP_LEAD, RING = 4 + LEAD;
     static_assert(!(BULK && ZBC), "the bulk-copy fetch path is built for periodic boundaries");
     static_assert(!(XCH && (ZBC || SPINOR)), "the exchanging strips are built for periodic scalar / reservoir grids");
-    static_assert(!(XCH && BULK && !step_ring_cpasync(sizeof(T) == 8, MODEL)), "exchanging strips take the cp.async flavour of the ring only");
+    static_assert(!(XCH && BULK && !step_ring_cpasync(sizeof(T) == 8, MODEL, VEC)), "exchanging strips take the cp.async flavour of the ring only");
     const Geom& g = a.geo;
     const Coef<T>& k = a.k;
     const int nx = g.nx, ny = g.ny;
@@ -489,7 +489,7 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
     // ---- bulk-copy fetch path: the ring, its mbarriers and the issuer's state ------------------------------------------------
     using SM = StepSmem<T, VEC, MODEL, DRIVE>;
     constexpr int DEPTH = (int)SM::DEPTH;
-    constexpr bool CPA = step_ring_cpasync(sizeof(T) == 8, MODEL);      // flavour of the ring: cp.async per lane, or TMA bulk copies
+    constexpr bool CPA = step_ring_cpasync(sizeof(T) == 8, MODEL, VEC);      // flavour of the ring: cp.async per lane, or TMA bulk copies
     extern __shared__ __align__(128) unsigned char step_smem[];
     uint32_t bar0 = 0, ring0 = 0;                       // shared-window addresses of this warp's mbarriers and stages
     const unsigned char* ringp = nullptr;

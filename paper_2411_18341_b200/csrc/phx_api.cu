@@ -398,7 +398,8 @@ double step_plan_cost(const phx_grid* g, int vec, int wpc, int* ly_out, bool xch
     const long slots = xch ? (long)g->n_sm * stepx_occupancy(g, vec, wpc)
                            : (long)g->n_sm * step_occupancy(g, vec) * (PHX_STEP_WARPS / wpc);   // resident CTAs of wpc warps
     const bool in_l2 = plane_cells(g) * g->d.batch * step_bytes_per_cell(g) < g->l2_bytes / 2;
-    const bool whole_passes = xch || step_bulk(g) || !step_early_exit(g->d.prec == PHX_C64, g->d.model, vec);
+    const bool whole_passes = xch || (step_bulk(g) && !step_ring_cpasync(g->d.prec == PHX_C64, g->d.model, vec)) ||
+                              !step_early_exit(g->d.prec == PHX_C64, g->d.model, vec);
     const int ring = xch ? 4 + step_xch_lead(g->d.prec == PHX_C64, g->d.model, vec) : PHX_STEP_RING;
     double best_cost = -1;
     int best_ly = g->d.ny;

@@ -58,8 +58,11 @@ namespace phx {
 // (slower than the register loads everywhere: profiles/r02_tma_vs_register_fetch.md).
 // (vec = cells per lane.)  The scalar fp32 kernel with 2 or 1 cells per lane gains 2-3 % as well (1024^2 116.2 against 113.4,
 // 1536^2 163.8 against 158.6); with 4 cells per lane it loses 11 % and keeps register loads (its ring, the TMA flavour, is opt-in).
+#ifndef PHX_RING_CPA_V4
+#define PHX_RING_CPA_V4 0
+#endif
 constexpr bool step_ring_cpasync(bool prec64, int model, int vec) {
-    return (!prec64 && model == 1) || (prec64 && model == 0) || (!prec64 && model == 0 && vec <= 2);
+    return (!prec64 && model == 1) || (prec64 && model == 0) || (!prec64 && model == 0 && (vec <= 2 || PHX_RING_CPA_V4));
 }
 constexpr int step_ring_depth(bool prec64, int model) { return (prec64 && model == 0) ? 4 : PHX_STEP_DEPTH; }
 constexpr bool step_ring_auto(bool prec64, int model, int vec) { return step_ring_cpasync(prec64, model, vec) && (vec == 2 || (prec64 && vec == 1)); }

@@ -169,6 +169,43 @@ template <int BYTES> __device__ __forceinline__ void cpasync(uint32_t dst, const
     }
 }
 
+// A lane's complex cells in the cp.async ring.  PHX_RING_PLANE = 16: a lane's 16-byte chunks sit next to each other (lane
+// stride 32 bytes when a lane holds 4 cells fp32 / 2 cells fp64).  PHX_RING_PLANE = 512 stores the row as planes of 16-byte
+// chunks (chunk h of lane l at row + h * 512 + l * 16) so that the 128-bit shared accesses of a warp are contiguous:
+// measured SLOWER (cfg2 4096^2 fp64 91.7 against 102.6-103.3 Gcell*step/s in the same run), so it is off.
+#ifndef PHX_RING_PLANE
+#define PHX_RING_PLANE 16
+#endif
+// The cp.async kernels may leave the row loop early like the register-load kernels (measured neutral).
+#ifndef PHX_RING_EXIT
+#define PHX_RING_EXIT 1
+#endif
+template <int BYTES> __device__ __forceinline__ void ring_cp(uint32_t row, int lane, const void* src) {
+    if constexpr (BYTES > 16) {
+#pragma unroll
+        for (int h = 0; h < BYTES / 16; ++h)
+            asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(row + h * PHX_RING_PLANE + lane * (PHX_RING_PLANE == 512 ? 16 : BYTES) + (PHX_RING_PLANE == 512 ? 0 : 0)), "l"(static_cast<const char*>(src) + h * 16) : "memory");
+    } else cpasync<BYTES>(row + lane * BYTES, src);
+}
+template <int VEC> __device__ __forceinline__ void ring_ld(const unsigned char* row, int lane, float2 (&v)[VEC]) {
+    if constexpr (VEC == 4) {
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+            const float4 q = *reinterpret_cast<const float4*>(row + h * PHX_RING_PLANE + lane * (PHX_RING_PLANE == 512 ? 16 : 32));
+            v[2 * h] = make_float2(q.x, q.y);
+            v[2 * h + 1] = make_float2(q.z, q.w);
+        }
+    } else if constexpr (VEC == 2) {
+        const float4 q = *reinterpret_cast<const float4*>(row + lane * 16);
+        v[0] = make_float2(q.x, q.y);
+        v[1] = make_float2(q.z, q.w);
+    } else v[0] = *reinterpret_cast<const float2*>(row + lane * 8);
+}
+template <int VEC> __device__ __forceinline__ void ring_ld(const unsigned char* row, int lane, double2 (&v)[VEC]) {
+#pragma unroll
+    for (int h = 0; h < VEC; ++h) v[h] = *reinterpret_cast<const double2*>(row + h * PHX_RING_PLANE + lane * (PHX_RING_PLANE == 512 ? 16 : 16 * VEC));
+}
+
 template <int VEC> __device__ __forceinline__ void ldsc(const float2* p, float2 (&v)[VEC]) {
     if constexpr (VEC % 2 == 0) {
 #pragma unroll
@@ -527,12 +564,12 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
             const uint32_t eq = (uint32_t)qi * (uint32_t)nx + (uint32_t)xg, ep = (uint32_t)qip * (uint32_t)nx + (uint32_t)xg;
 #pragma unroll
             for (int s = 0; s < NC; ++s) {
-                cpasync<VEC * sizeof(C)>(dst + SM::PSI + (s * W + lane * VEC) * sizeof(C), pin[s] + eq);
+                ring_cp<VEC * sizeof(C)>(dst + SM::PSI + s * W * sizeof(C), lane, pin[s] + eq);
                 if constexpr (RES) cpasync<VEC * sizeof(T)>(dst + SM::N + (s * W + lane * VEC) * sizeof(T), nin[s] + ep);
             }
             if (Vp) cpasync<VEC * sizeof(T)>(dst + SM::V + lane * VEC * sizeof(T), Vp + ep);
             if (Pp) cpasync<VEC * sizeof(T)>(dst + SM::P + lane * VEC * sizeof(T), Pp + ep);
-            if constexpr (DRIVE) cpasync<VEC * sizeof(C)>(dst + SM::E + lane * VEC * sizeof(C), Ep + ep);
+            if constexpr (DRIVE) ring_cp<VEC * sizeof(C)>(dst + SM::E, lane, Ep + ep);
             asm volatile("cp.async.commit_group;" ::: "memory");
             ++fi;
             qip = qi;
@@ -577,7 +614,7 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
 #pragma unroll
         for (int ph = 0; ph < RING; ++ph) {
             const int j = jb + ph;          // front row of this iteration
-            if constexpr (!BULK && !XCH && step_early_exit(sizeof(T) == 8, MODEL, VEC)) {
+            if constexpr ((!BULK || (PHX_RING_EXIT && step_ring_cpasync(sizeof(T) == 8, MODEL, VEC))) && !XCH && step_early_exit(sizeof(T) == 8, MODEL, VEC)) {
                 if (ph > 0 && j > r1 + 2) break;   // (warp-uniform) the chunk is done: row r1-1 was stored in the iteration with front row r1+2
             }
             C xin[4];                       // (XCH) the neighbours' cells next to this lane's strip: of psi[j], y2[j-1], y3[j-2], y4[j-3]
@@ -635,12 +672,16 @@ step_kernel(const __grid_constant__ StepArgs<T> a) {
                 const unsigned char* st = ringp + slot * SM::STAGE;
 #pragma unroll
                 for (int s = 0; s < NC; ++s) {
-                    ldsc<VEC>(reinterpret_cast<const C*>(st + SM::PSI) + s * W + lane * VEC, psr[s][SL(1 + LEAD)]);
+                    if constexpr (CPA) ring_ld<VEC>(st + SM::PSI + s * W * sizeof(C), lane, psr[s][SL(1 + LEAD)]);
+                    else ldsc<VEC>(reinterpret_cast<const C*>(st + SM::PSI) + s * W + lane * VEC, psr[s][SL(1 + LEAD)]);
                     if constexpr (RES) ldsr<VEC>(reinterpret_cast<const T*>(st + SM::N) + s * W + lane * VEC, nr[s][SL(LEAD)]);
                 }
                 if (Vp) ldsr<VEC>(reinterpret_cast<const T*>(st + SM::V) + lane * VEC, Vr[SL(LEAD)]);
                 if (Pp) ldsr<VEC>(reinterpret_cast<const T*>(st + SM::P) + lane * VEC, Pr[SL(LEAD)]);
-                if constexpr (DRIVE) ldsc<VEC>(reinterpret_cast<const C*>(st + SM::E) + lane * VEC, Er[SL(LEAD)]);
+                if constexpr (DRIVE) {
+                    if constexpr (CPA) ring_ld<VEC>(st + SM::E, lane, Er[SL(LEAD)]);
+                    else ldsc<VEC>(reinterpret_cast<const C*>(st + SM::E) + lane * VEC, Er[SL(LEAD)]);
+                }
                 ++fc;
                 if constexpr (!CPA) ready = mbar_test(bar0 + ((uint32_t)fc % DEPTH) * 8, ((uint32_t)fc / DEPTH) & 1u);
             } else {

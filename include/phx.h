@@ -214,7 +214,7 @@ phx_status phx_select_variant(phx_grid* g, int32_t variant);
  * "step_warps" (warps per CTA), "step_xch" (exchanging strips: -1 automatic, 0 off, 1 wherever the row is 1-8 strips wide),
  * "step_bulk" (1: rows fetched by TMA bulk copies into shared memory), "step_side" (1: side launch for a ragged last strip),
  * "step_pdl" (later steps of a graph as programmatic dependent launches: -1 automatic, 0 off, 1 on),
- * "resident_cluster" (variant RESIDENT on a thread-block cluster of 2-8 CTAs: -1 automatic, 0 never, 1 wherever it applies),
+ * "resident_cluster" (variant RESIDENT on a thread-block cluster of 2-16 CTAs: -1 automatic, 0 never, 1 wherever it applies),
  * "graph_steps" (RK4 steps per captured CUDA graph).  Results do not depend on them (bit for bit within variant STEP).
  * "async_host_copies" = 1: phx_set_field / phx_read_field with PHX_HOST enqueue the copy on the stream and return
  * without synchronising (the host buffers must be pinned and stay untouched until phx_sync); lets a caller overlap the

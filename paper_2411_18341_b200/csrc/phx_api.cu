@@ -630,9 +630,9 @@ bool resident_variant_ok(const phx_grid* g) {
     return resident_single_ok(g) || (g->resident_cluster != 0 && resident_cluster_ctas(g) != 0);
 }
 
-// Largest single grid AUTO gives to the cluster form of variant RESIDENT (measured, us per step, cluster form against the fused
-// step: cfg1 64^2 fp64 2.45 / 3.58, 64^2 fp32 2.08 / 3.33, 128^2 fp32 4.91 / 3.38, 128^2 fp64 5.72 / 3.92).
-constexpr int RESIDENT_CLUSTER_AUTO_CELLS = 4096;
+// Largest single grid AUTO gives to the cluster form of variant RESIDENT (measured, us per step, clusters of 16 CTAs against the
+// fused step: cfg1 64^2 fp64 2.23 / 3.58, 64^2 fp32 1.74 / 3.33, 128^2 fp32 2.92 / 3.38, 128^2 fp64 3.53 / 3.92).
+constexpr int RESIDENT_CLUSTER_AUTO_CELLS = 16384;
 
 // AUTO takes the resident kernel for ensembles of grids that fit it (one CTA per realisation: 2.3x the fused step on
 // 512 x 64^2 fp32; a single small grid is faster spread over several SMs by the fused step: 3.9 against 4.3 us per step at
@@ -641,7 +641,7 @@ constexpr int RESIDENT_CLUSTER_AUTO_CELLS = 4096;
 void resolve_variant(phx_grid* g) {
     const int req = g->variant_req;
     const bool res_ok = resident_variant_ok(g);
-    // (AUTO: ensembles of grids that fit one CTA; single grids of at most 4096 cells on a cluster, one cell per thread)
+    // (AUTO: ensembles of grids that fit one CTA; single grids of at most 128^2 cells on a cluster)
     const bool auto_res = g->d.batch >= 32 ? resident_single_ok(g)
                                            : (resident_use_cluster(g) && plane_cells(g) <= (size_t)RESIDENT_CLUSTER_AUTO_CELLS);
     if (res_ok && (req == PHX_VARIANT_RESIDENT || (req == PHX_VARIANT_AUTO && auto_res))) g->variant = PHX_VARIANT_RESIDENT;

@@ -11,7 +11,7 @@
 // last.  Scalar and reservoir models, both precisions, optional noise (Eq. (22)); no drive.
 // The derivative is the one of variant STEP (phx_deriv.cuh).  Product code: shares nothing with oracle/.
 //
-// CLUSTER form (resident_cluster_kernel): one realisation spread over a thread-block cluster of 2-8 CTAs, each owning a slab
+// CLUSTER form (resident_cluster_kernel): one realisation spread over a thread-block cluster of 2-16 CTAs, each owning a slab
 // of ny / cluster rows plus one halo row above and below in its own shared memory.  After a stage every CTA stores the first
 // and last row it produced straight into its neighbours' halo rows through distributed shared memory
 // (cluster.map_shared_rank), then the cluster barrier (barrier.cluster, ~380 cycles) takes the place of __syncthreads.  For a
@@ -28,6 +28,9 @@
 namespace phx {
 
 constexpr int RES_NT = PHX_RESIDENT_THREADS;
+#ifndef PHX_RESIDENT_MAX_CLUSTER
+#define PHX_RESIDENT_MAX_CLUSTER 16     // (beyond 8: the non-portable cluster size attribute, set at launch)
+#endif
 
 template <typename T, bool RES, bool NOISE, int CPT>
 __global__ void __launch_bounds__(RES_NT, 1)
@@ -161,7 +164,7 @@ resident_cluster_kernel(const __grid_constant__ ResidentArgs<T> a) {
     T* Vs = reinterpret_cast<T*>(nbr + NL);
     T* Ps = Vs + NL;
 
-    const int tid = threadIdx.x;
+    const int tid = threadIdx.x, nt = blockDim.x;      // (a slab smaller than the largest CTA runs with fewer threads)
     const int real = blockIdx.x / ncta;
     const size_t boff = (size_t)real * g.plane;
     C* psi_g = a.psi + boff;
@@ -174,13 +177,13 @@ resident_cluster_kernel(const __grid_constant__ ResidentArgs<T> a) {
     C* rs0 = cluster.map_shared_rank(buf0, rank_s); C* rs1 = cluster.map_shared_rank(buf1, rank_s);
     C* rn0 = cluster.map_shared_rank(buf0, rank_n); C* rn1 = cluster.map_shared_rank(buf1, rank_n);
 
-    for (int c = tid; c < NB + 1; c += RES_NT) { buf0[c] = czero; buf1[c] = czero; }
+    for (int c = tid; c < NB + 1; c += nt) { buf0[c] = czero; buf1[c] = czero; }
     __syncthreads();
     C psi[CPT], acc[CPT];
     T nn[CPT], nacc[CPT], nst[CPT];
 #pragma unroll
     for (int q = 0; q < CPT; ++q) {
-        const int c = tid + q * RES_NT;
+        const int c = tid + q * nt;
         psi[q] = czero; acc[q] = czero; nn[q] = T(0); nacc[q] = T(0); nst[q] = T(0);
         if (c < NL) {
             const int lr = c / nx, i = c - lr * nx, b = (lr + 1) * nx + i;
@@ -197,7 +200,7 @@ resident_cluster_kernel(const __grid_constant__ ResidentArgs<T> a) {
         }
     }
     // halo rows of the first stage input, from global memory
-    for (int i = tid; i < nx; i += RES_NT) {
+    for (int i = tid; i < nx; i += nt) {
         if (has_s) buf0[i] = psi_g[(size_t)(j0 == 0 ? g.ny - 1 : j0 - 1) * nx + i];
         if (has_n) buf0[(rl + 1) * nx + i] = psi_g[(size_t)(j0 + rl == g.ny ? 0 : j0 + rl) * nx + i];
     }
@@ -209,7 +212,7 @@ resident_cluster_kernel(const __grid_constant__ ResidentArgs<T> a) {
         const T w_dt = (s == 1 || s == 4) ? k.dt6 : k.dt3;
 #pragma unroll
         for (int q = 0; q < CPT; ++q) {
-            const int c = tid + q * RES_NT;
+            const int c = tid + q * nt;
             if (c < NL) {
                 const int lr = c / nx, i = c - lr * nx, b = (lr + 1) * nx + i;
                 const ushort2 nb = nbr[c];
@@ -261,7 +264,7 @@ resident_cluster_kernel(const __grid_constant__ ResidentArgs<T> a) {
 
 #pragma unroll
     for (int q = 0; q < CPT; ++q) {
-        const int c = tid + q * RES_NT;
+        const int c = tid + q * nt;
         if (c < NL) {
             const int lr = c / nx, i = c - lr * nx;
             const size_t gc = (size_t)(j0 + lr) * nx + i;
@@ -280,11 +283,11 @@ size_t resident_cluster_smem_bytes(int nx, int rl, int prec64) {
     return 2 * nb * 2 * rb + nl * sizeof(ushort2) + 2 * nl * rb;
 }
 
-// Cluster size for one realisation of an nx x ny grid (0 = the cluster form does not apply): the largest of 8, 4, 2 that
+// Cluster size for one realisation of an nx x ny grid (0 = the cluster form does not apply): the largest of 16, 8, 4, 2 that
 // divides ny, gives every CTA at least 2 rows, and whose slab fits 4 cells per thread and the shared memory.
 int resident_cluster_size(int nx, int ny, int prec64, bool res) {
     (void)res;
-    for (int n = 8; n >= 2; n >>= 1) {
+    for (int n = PHX_RESIDENT_MAX_CLUSTER; n >= 2; n >>= 1) {
         if (ny % n != 0 || ny / n < 2) continue;
         const int rl = ny / n;
         if ((size_t)rl * nx > 4u * RES_NT || (size_t)(rl + 2) * nx + 1 > 65535u) continue;
@@ -300,9 +303,14 @@ static cudaError_t launch_cluster_one(const ResidentArgs<T>& a, int ncta, cudaSt
     auto kern = resident_cluster_kernel<T, RES, NOISE, CPT>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
+    if (ncta > 8) {
+        e = cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
+        if (e != cudaSuccess) return e;
+    }
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3((unsigned)(a.geo.batch * ncta));
-    cfg.blockDim = dim3(RES_NT);
+    const int nl = a.geo.nx * (a.geo.ny / ncta);
+    cfg.blockDim = dim3(CPT == 1 ? (unsigned)((nl + 31) / 32 * 32) : (unsigned)RES_NT);   // one cell per thread: no idle warps at the barriers
     cfg.dynamicSmemBytes = smem;
     cfg.stream = st;
     cudaLaunchAttribute attr[1];

@@ -130,7 +130,7 @@ def test_grids_that_do_not_fit_are_refused():
     g.destroy()
 
 
-# ---- cluster form: one realisation on a thread-block cluster of 2-8 CTAs ------------------------------
+# ---- cluster form: one realisation on a thread-block cluster of 2-16 CTAs ------------------------------
 @pytest.mark.parametrize("maker,bc", [
     (lambda: wl.cfg1(n_steps=100), (0, 0)),                               # 64 x 64 fp64: 8 CTAs of 8 rows, one cell per thread
     (lambda: wl.cfg2(n=64, ny=64, prec="c32"), (0, 0)),
@@ -169,10 +169,13 @@ def test_cluster_form(maker, bc):
 
 
 def test_cluster_form_opens_resident_to_128_wide_grids():
-    g = make_gpu(wl.cfg2(n=128, ny=128, prec="c32"))      # AUTO: the fused step (faster at this size)
+    g = make_gpu(wl.cfg2(n=128, ny=128, prec="c32"))      # AUTO: does not fit one CTA; a cluster of 16 steps it faster than STEP
+    assert g.get_variant() == RESIDENT
+    g.destroy()
+    g = make_gpu(wl.cfg2(n=192, ny=96, prec="c32"))       # AUTO beyond 128^2 cells: the fused step
     assert g.get_variant() == STEP
     g.select_variant(RESIDENT)
-    assert g.get_variant() == RESIDENT                     # does not fit one CTA: the cluster form
+    assert g.get_variant() == RESIDENT                     # (the cluster form, on request)
     g.destroy()
     g = make_gpu(wl.cfg2(n=128, ny=128, prec="c32"), tuning={"resident_cluster": 0})
     with pytest.raises(phx.PhxError):

@@ -28,6 +28,10 @@
 namespace phx {
 
 constexpr int RES_NT = PHX_RESIDENT_THREADS;
+// Scalar grids on a cluster: two stages per cluster barrier (resident_pair_kernel) instead of one.
+#ifndef PHX_RESIDENT_PAIR
+#define PHX_RESIDENT_PAIR 1
+#endif
 #ifndef PHX_RESIDENT_MAX_CLUSTER
 #define PHX_RESIDENT_MAX_CLUSTER 16     // (beyond 8: the non-portable cluster size attribute, set at launch)
 #endif
@@ -323,10 +327,221 @@ static cudaError_t launch_cluster_one(const ResidentArgs<T>& a, int ncta, cudaSt
     return cudaLaunchKernelEx(&cfg, kern, a);
 }
 
+
+// ---- cluster form, two stages per cluster barrier (scalar model) ----------------------------------------------------------
+// As resident_cluster_kernel, but every CTA also computes the odd stages (1 and 3) on ONE extra row above and below its slab
+// (the paper's shrinking halo, in rows: redundant arithmetic instead of a barrier), so that a cluster barrier
+// is needed only after the even stages: two per RK4 step instead of four, with two halo rows exchanged each time.
+// Local rows r = -2 .. rl+1 (buffer row r + 2); threads own the cells of rows -1 .. rl ("extended slab"); three stage buffers
+// A, B, C rotate so that no CTA writes into a neighbour's buffer that the neighbour may still be reading:
+//   S1: A -> B on rows -1 .. rl      __syncthreads      S2: B -> C on rows 0 .. rl-1, edge rows pushed into the neighbours' C
+//   cluster barrier
+//   S3: C -> B on rows -1 .. rl      __syncthreads      S4: B -> A on rows 0 .. rl-1 (psi(t+dt)), edge rows pushed into A
+//   cluster barrier
+template <typename T, bool NOISE, int CPT>
+__global__ void __launch_bounds__(RES_NT, 1)
+resident_pair_kernel(const __grid_constant__ ResidentArgs<T> a) {
+    namespace cg = cooperative_groups;
+    using C = typename Cx<T>::type;
+    extern __shared__ __align__(16) unsigned char smem[];
+    cg::cluster_group cluster = cg::this_cluster();
+    const Geom& g = a.geo;
+    const Coef<T>& k = a.k;
+    const int ncta = (int)cluster.num_blocks(), rank = (int)cluster.block_rank();
+    const int nx = g.nx, ny = g.ny, rl = ny / ncta, NE = (rl + 2) * nx, NB = (rl + 4) * nx;    // NB = index of the zero cell
+    C* bufA = reinterpret_cast<C*>(smem);
+    C* bufB = bufA + (NB + 1);
+    C* bufC = bufB + (NB + 1);
+    ushort2* nbr = reinterpret_cast<ushort2*>(bufC + (NB + 1));                   // west, east
+    T* Vs = reinterpret_cast<T*>(nbr + NE);
+
+    const int tid = threadIdx.x, nt = blockDim.x;
+    const int real = blockIdx.x / ncta;
+    const size_t boff = (size_t)real * g.plane;
+    C* psi_g = a.psi + boff;
+    const C czero = mk<T>(T(0), T(0));
+    const int j0 = rank * rl;
+    const bool has_s = !(g.bc_y && rank == 0), has_n = !(g.bc_y && rank == ncta - 1);
+    const int rank_s = rank == 0 ? ncta - 1 : rank - 1, rank_n = rank == ncta - 1 ? 0 : rank + 1;
+    C* sA = cluster.map_shared_rank(bufA, rank_s); C* sC = cluster.map_shared_rank(bufC, rank_s);
+    C* nA = cluster.map_shared_rank(bufA, rank_n); C* nC = cluster.map_shared_rank(bufC, rank_n);
+    // global row of local row r (wrapped); -1 = outside a zero boundary
+    auto grow = [&](int r) {
+        int j = j0 + r;
+        if (j < 0 || j >= ny) {
+            if (g.bc_y) return -1;
+            j = j < 0 ? j + ny : j - ny;
+        }
+        return j;
+    };
+
+    for (int c = tid; c < 3 * (NB + 1); c += nt) bufA[c] = czero;       // (the three buffers are contiguous)
+    __syncthreads();
+    C psi[CPT], acc[CPT];
+    bool own[CPT], live[CPT];       // own: a cell of the slab; live: a cell of the extended slab inside the domain
+#pragma unroll
+    for (int q = 0; q < CPT; ++q) {
+        const int c = tid + q * nt;
+        psi[q] = czero; acc[q] = czero; own[q] = false; live[q] = false;
+        if (c < NE) {
+            const int er = c / nx, i = c - er * nx, b = (er + 1) * nx + i, j = grow(er - 1);
+            own[q] = er >= 1 && er <= rl;
+            live[q] = j >= 0;
+            ushort2 nb;
+            nb.x = (unsigned short)(i > 0 ? b - 1 : (g.bc_x ? NB : b + nx - 1));
+            nb.y = (unsigned short)(i < nx - 1 ? b + 1 : (g.bc_x ? NB : b - nx + 1));
+            nbr[c] = nb;
+            Vs[c] = (a.V && j >= 0) ? a.V[(size_t)j * nx + i] : T(0);
+            if (j >= 0) { psi[q] = psi_g[(size_t)j * nx + i]; bufA[b] = psi[q]; }
+        }
+    }
+    for (int i = tid; i < nx; i += nt) {        // the outer halo rows -2 and rl+1 of the first stage input
+        const int js = grow(-2), jn = grow(rl + 1);
+        if (js >= 0) bufA[i] = psi_g[(size_t)js * nx + i];
+        if (jn >= 0) bufA[(rl + 3) * nx + i] = psi_g[(size_t)jn * nx + i];
+    }
+    (void)has_s; (void)has_n;
+    cluster.sync();
+
+    auto odd_stage = [&](const C* in, C* out, auto stage_no) {          // stages 1 and 3, on the extended slab
+        constexpr int s = decltype(stage_no)::value;
+        const T a_dt = s == 3 ? k.dt : k.hdt;
+        const T w_dt = s == 1 ? k.dt6 : k.dt3;
+#pragma unroll
+        for (int q = 0; q < CPT; ++q) {
+            const int c = tid + q * nt;
+            if (c < NE && live[q]) {
+                const int er = c / nx, i = c - er * nx, b = (er + 1) * nx + i;
+                const ushort2 nb = nbr[c];
+                Nbhd<T> h;
+                h.c = s == 1 ? psi[q] : in[b];
+                h.w = in[nb.x]; h.e = in[nb.y]; h.s = in[b - nx]; h.n = in[b + nx];
+                Diff<T> df;
+                differences<T, false, false>(k, h, df);
+                T Kn;
+                const C K = deriv<T, false, false, false>(k, h.c, df, czero, df, true, T(0), Vs[c], T(0), czero, czero, Kn);
+                if (own[q]) acc[q] = fma2s(w_dt, K, s == 1 ? psi[q] : acc[q]);
+                out[b] = fma2s(a_dt, K, psi[q]);
+            }
+        }
+        __syncthreads();
+    };
+    auto even_stage = [&](const C* in, C* out, C* out_s, C* out_n, auto stage_no, const uint64_t step) {   // stages 2 and 4, on the slab
+        constexpr int s = decltype(stage_no)::value;
+#pragma unroll
+        for (int q = 0; q < CPT; ++q) {
+            const int c = tid + q * nt;
+            if (c < NE && own[q]) {
+                const int er = c / nx, i = c - er * nx, b = (er + 1) * nx + i, r = er - 1;
+                const ushort2 nb = nbr[c];
+                Nbhd<T> h;
+                h.c = in[b];
+                h.w = in[nb.x]; h.e = in[nb.y]; h.s = in[b - nx]; h.n = in[b + nx];
+                Diff<T> df;
+                differences<T, false, false>(k, h, df);
+                T Kn;
+                const C K = deriv<T, false, false, false>(k, h.c, df, czero, df, true, T(0), Vs[c], T(0), czero, czero, Kn);
+                C y;
+                if (s == 2) {
+                    acc[q] = fma2s(k.dt3, K, acc[q]);
+                    y = fma2s(k.hdt, K, psi[q]);
+                } else {
+                    y = fma2s(k.dt6, K, acc[q]);
+                    if (NOISE) {
+                        const uint4 wd = noise_words(a.seed, (uint32_t)real, step, (uint32_t)((j0 + r) * nx + i));
+                        y = add2(y, noise_increment_sfu(wd.x, wd.y, k.sig2 * (T(2) * k.hgc)));
+                    }
+                    psi[q] = y;
+                }
+                out[b] = y;
+                // the two first rows of the slab are rows rl, rl+1 of the CTA below; the two last rows are rows -2, -1 of the CTA above
+                if (r < 2 && has_s) out_s[(rl + r + 2) * nx + i] = y;
+                if (r >= rl - 2 && has_n) out_n[(r - rl + 2) * nx + i] = y;
+            }
+        }
+        cluster.sync();
+    };
+
+    for (int it = 0; it < a.n_steps; ++it) {
+        const uint64_t step = a.step0 + (uint64_t)it;
+        if (it > 0) {           // the cells of the extra rows take psi(t) from what the neighbours pushed
+#pragma unroll
+            for (int q = 0; q < CPT; ++q) {
+                const int c = tid + q * nt;
+                if (c < NE && live[q] && !own[q]) psi[q] = bufA[(c / nx + 1) * nx + c % nx];
+            }
+        }
+        odd_stage(bufA, bufB, std::integral_constant<int, 1>());
+        even_stage(bufB, bufC, sC, nC, std::integral_constant<int, 2>(), step);
+        odd_stage(bufC, bufB, std::integral_constant<int, 3>());
+        even_stage(bufB, bufA, sA, nA, std::integral_constant<int, 4>(), step);
+    }
+
+#pragma unroll
+    for (int q = 0; q < CPT; ++q) {
+        const int c = tid + q * nt;
+        if (c < NE && own[q]) {
+            const int er = c / nx, i = c - er * nx;
+            psi_g[(size_t)(j0 + er - 1) * nx + i] = psi[q];
+        }
+    }
+    if (blockIdx.x == 0 && tid == 0) {
+        a.step_slots[0] = a.step0 + (uint64_t)a.n_steps;
+        a.step_slots[1] = a.step0 + (uint64_t)a.n_steps;
+    }
+}
+
+size_t resident_pair_smem_bytes(int nx, int rl, int prec64) {
+    const size_t rb = prec64 ? 8 : 4, nb = (size_t)(rl + 4) * nx + 1, ne = (size_t)(rl + 2) * nx;
+    return 3 * nb * 2 * rb + ne * sizeof(ushort2) + ne * rb;
+}
+
+// The pair kernel applies to the scalar model when the extended slab fits 4 cells per thread.
+bool resident_pair_ok(int nx, int ny, int ncta, int prec64) {
+    if (ncta < 2 || ny % ncta != 0) return false;
+    const int rl = ny / ncta;
+    if (rl < 2 || (size_t)(rl + 2) * nx > 4u * RES_NT || (size_t)(rl + 4) * nx + 1 > 65535u) return false;
+    return resident_pair_smem_bytes(nx, rl, prec64) <= 200 * 1024;
+}
+
+template <typename T, bool NOISE, int CPT>
+static cudaError_t launch_pair_one(const ResidentArgs<T>& a, int ncta, cudaStream_t st) {
+    const int rl = a.geo.ny / ncta, ne = (rl + 2) * a.geo.nx;
+    const size_t smem = resident_pair_smem_bytes(a.geo.nx, rl, sizeof(T) == 8);
+    auto kern = resident_pair_kernel<T, NOISE, CPT>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    if (ncta > 8) {
+        e = cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
+        if (e != cudaSuccess) return e;
+    }
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)(a.geo.batch * ncta));
+    cfg.blockDim = dim3(CPT == 1 ? (unsigned)((ne + 31) / 32 * 32) : (unsigned)RES_NT);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = (unsigned)ncta;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kern, a);
+}
+
+template <typename T>
+static cudaError_t launch_pair_t(const ResidentArgs<T>& a, bool noise, int ncta, cudaStream_t st) {
+    const int need = ((a.geo.ny / ncta + 2) * a.geo.nx + RES_NT - 1) / RES_NT;
+    if (noise) return need == 1 ? launch_pair_one<T, true, 1>(a, ncta, st) : launch_pair_one<T, true, 4>(a, ncta, st);
+    return need == 1 ? launch_pair_one<T, false, 1>(a, ncta, st) : launch_pair_one<T, false, 4>(a, ncta, st);
+}
+
 template <typename T>
 static cudaError_t launch_cluster_t(const ResidentArgs<T>& a, bool res, bool noise, cudaStream_t st) {
     const int ncta = resident_cluster_size(a.geo.nx, a.geo.ny, sizeof(T) == 8, res);
     if (ncta == 0) return cudaErrorInvalidConfiguration;
+    if (PHX_RESIDENT_PAIR && !res && resident_pair_ok(a.geo.nx, a.geo.ny, ncta, sizeof(T) == 8)) return launch_pair_t<T>(a, noise, ncta, st);
     const int need = (a.geo.nx * (a.geo.ny / ncta) + RES_NT - 1) / RES_NT;
 #define PHX_RESC_CASE(R, NZ)                                                  \
     if (res == R && noise == NZ) {                                            \

@@ -130,6 +130,12 @@ def test_grids_that_do_not_fit_are_refused():
     g.destroy()
 
 
+def _noisy(w):
+    w.noise, w.seed = True, 13
+    w.params = dict(w.params, noise_scale=1e-6)
+    return w
+
+
 # ---- cluster form: one realisation on a thread-block cluster of 2-16 CTAs ------------------------------
 @pytest.mark.parametrize("maker,bc", [
     (lambda: wl.cfg1(n_steps=100), (0, 0)),                               # 64 x 64 fp64: 8 CTAs of 8 rows, one cell per thread
@@ -142,7 +148,9 @@ def test_grids_that_do_not_fit_are_refused():
     (lambda: wl.cfg3(n=64, prec="c32"), (0, 0)),
     (lambda: wl.cfg3(n=128, prec="c64"), (0, 0)),
     (lambda: wl.cfg5(n=64, batch=3, prec="c32"), (0, 0)),                 # noise: the cell index of the counter is the grid's
-    (lambda: wl.cfg5(n=128, batch=2, prec="c32"), (0, 0))])
+    (lambda: wl.cfg5(n=128, batch=2, prec="c32"), (0, 0)),
+    (lambda: _noisy(wl.cfg2(n=64, ny=64, prec="c32")), (0, 0)),           # scalar + noise: the two-stages-per-barrier kernel
+    (lambda: _noisy(wl.cfg2(n=40, ny=24, prec="c64")), (1, 1))])
 def test_cluster_form(maker, bc):
     w = maker()
     g = make_gpu(w, variant=RESIDENT, bc=bc, tuning={"resident_cluster": 1})
@@ -153,6 +161,7 @@ def test_cluster_form(maker, bc):
     o.step_rk4(61)
     compare(g, o, w)
     assert g.get_launch_count() == 2 and g.get_step() == 61
+    # (scalar grids run resident_pair_kernel: two stages per cluster barrier, one redundant row of arithmetic on either side)
     # against the one-CTA form where the grid fits it: the same cell arithmetic (phx_deriv.cuh), hence the same bits -- except
     # with noise, where the compiler contracts the reservoir / variance expressions differently for 1 and 8 cells per thread
     # (rounding-level: bounded at a tenth of the field tolerance)

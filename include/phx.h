@@ -212,7 +212,8 @@ phx_status phx_select_variant(phx_grid* g, int32_t variant);
  * launch geometry knobs (key/value, UNSUPPORTED for unknown keys): "rows", "vec" (variant STAGE: rows per
  * CTA, cells per thread), "step_ly", "step_vec" (variant STEP: rows per chunk, cells per lane; 0 = automatic),
  * "step_warps" (warps per CTA), "step_xch" (exchanging strips: -1 automatic, 0 off, 1 wherever the row is 1-8 strips wide),
- * "step_bulk" (1: rows fetched by TMA bulk copies into shared memory), "step_side" (1: side launch for a ragged last strip),
+ * "step_bulk" (rows fetched through a shared-memory ring, by per-lane cp.async or by TMA bulk copies depending on the kernel:
+ * -1 automatic = where it measured faster, 0 register loads, 1 the ring), "step_side" (1: side launch for a ragged last strip),
  * "step_pdl" (later steps of a graph as programmatic dependent launches: -1 automatic, 0 off, 1 on),
  * "resident_cluster" (variant RESIDENT on a thread-block cluster of 2-16 CTAs: -1 automatic, 0 never, 1 wherever it applies),
  * "graph_steps" (RK4 steps per captured CUDA graph).  Results do not depend on them (bit for bit within variant STEP).

@@ -1200,7 +1200,7 @@ phx_status phx_set_tuning(phx_grid* g, const char* key, int32_t value) {
     } else if (!std::strcmp(key, "step_warps")) {     // variant STEP: warps per CTA (0 = automatic)
         if (value < 0 || value > PHX_STEP_WARPS) return PHX_ERR_INVALID_ARG;
         g->step_warps = value;
-    } else if (!std::strcmp(key, "step_bulk")) {      // variant STEP fetch path: -1 automatic, 0 register loads, 1 bulk copies
+    } else if (!std::strcmp(key, "step_bulk")) {      // variant STEP fetch path: -1 automatic, 0 register loads, 1 shared-memory ring (cp.async / TMA)
         if (value < -1 || value > 1) return PHX_ERR_INVALID_ARG;
         g->step_bulk = value;
     } else if (!std::strcmp(key, "step_xch")) {       // variant STEP exchanging strips: -1 automatic (wherever the row fits), 0 off

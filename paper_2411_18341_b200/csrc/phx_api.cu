@@ -569,6 +569,7 @@ int resident_cluster_ctas(const phx_grid* g) {
 bool resident_use_cluster(const phx_grid* g) {
     const int n = resident_cluster_ctas(g);
     if (n == 0 || g->resident_cluster == 0) return false;
+    if (g->hasE) return true;                                 // (a drive: only the cluster form of the scalar model carries it)
     if (!resident_single_ok(g) || g->resident_cluster == 1) return true;
     return (long)g->d.batch * n <= (long)g->n_sm;          // every cluster resident at once: more SMs per realisation
 }
@@ -585,6 +586,7 @@ cudaError_t launch_resident(phx_grid* g, int n_steps) {
     a.n = res ? (T*)(g->ws + (g->parity ? g->L.na[0] : g->L.n[0])) : nullptr;
     a.V = g->hasV ? (const T*)(g->ws + g->L.V) : nullptr;
     a.P = g->hasP ? (const T*)(g->ws + g->L.P) : nullptr;
+    a.E = g->hasE ? (const C*)(g->ws + g->L.E) : nullptr;
     a.step_slots = (uint64_t*)(g->ws + g->L.step);
     a.step0 = g->step_host;
     a.n_steps = n_steps;
@@ -626,7 +628,8 @@ bool step_variant_ok(const phx_grid* g) { return (size_t)g->d.nx * (size_t)g->d.
 
 // Variant RESIDENT: scalar and reservoir models without drive whose grid fits one CTA (phx_resident.cu).
 bool resident_variant_ok(const phx_grid* g) {
-    if (model_spinor(g->d.model) || g->hasE) return false;
+    if (model_spinor(g->d.model)) return false;
+    if (g->hasE) return g->d.model == PHX_SCALAR && g->resident_cluster != 0 && resident_drive_ok(g->d.nx, g->d.ny, g->d.prec == PHX_C64);
     return resident_single_ok(g) || (g->resident_cluster != 0 && resident_cluster_ctas(g) != 0);
 }
 

@@ -136,12 +136,14 @@ struct ResidentArgs {
     uint64_t step0;                 // completed steps before this launch
     int n_steps;
     uint32_t seed;
+    const typename Cx<T>::type* E;  // drive amplitude [ny][nx] or nullptr (cluster form of the scalar model only)
 };
 int resident_cpt(size_t cells, int prec64, bool res);     // cells per thread, 0 = the grid does not fit
 cudaError_t launch_resident_32(const ResidentArgs<float>&, bool res, bool noise, cudaStream_t);
 cudaError_t launch_resident_64(const ResidentArgs<double>&, bool res, bool noise, cudaStream_t);
 // cluster form: one realisation on a thread-block cluster of 2-8 CTAs (row slabs, halo rows through distributed shared memory)
 int resident_cluster_size(int nx, int ny, int prec64, bool res);   // 0 = does not apply
+bool resident_drive_ok(int nx, int ny, int prec64);                // a driven scalar grid fits the cluster form
 cudaError_t launch_resident_cluster_32(const ResidentArgs<float>&, bool res, bool noise, cudaStream_t);
 cudaError_t launch_resident_cluster_64(const ResidentArgs<double>&, bool res, bool noise, cudaStream_t);
 

@@ -165,7 +165,7 @@ resident_cluster_kernel(const __grid_constant__ ResidentArgs<T> a) {
     C* buf0 = reinterpret_cast<C*>(smem);
     C* buf1 = buf0 + (NB + 1);
     ushort2* nbr = reinterpret_cast<ushort2*>(buf1 + (NB + 1));                   // west, east (south / north are -+ nx)
-    T* Vs = reinterpret_cast<T*>(nbr + NL);
+    T* Vs = reinterpret_cast<T*>((reinterpret_cast<uintptr_t>(nbr + NL) + 15) & ~(uintptr_t)15);      // (an odd cell count: keep T aligned)
     T* Ps = Vs + NL;
 
     const int tid = threadIdx.x, nt = blockDim.x;      // (a slab smaller than the largest CTA runs with fewer threads)
@@ -284,7 +284,7 @@ resident_cluster_kernel(const __grid_constant__ ResidentArgs<T> a) {
 
 size_t resident_cluster_smem_bytes(int nx, int rl, int prec64) {
     const size_t rb = prec64 ? 8 : 4, nb = (size_t)(rl + 2) * nx + 1, nl = (size_t)rl * nx;
-    return 2 * nb * 2 * rb + nl * sizeof(ushort2) + 2 * nl * rb;
+    return 2 * nb * 2 * rb + nl * sizeof(ushort2) + 2 * nl * rb + 16;      // (+ alignment slack)
 }
 
 // Cluster size for one realisation of an nx x ny grid (0 = the cluster form does not apply): the largest of 16, 8, 4, 2 that
@@ -338,7 +338,8 @@ static cudaError_t launch_cluster_one(const ResidentArgs<T>& a, int ncta, cudaSt
 //   cluster barrier
 //   S3: C -> B on rows -1 .. rl      __syncthreads      S4: B -> A on rows 0 .. rl-1 (psi(t+dt)), edge rows pushed into A
 //   cluster barrier
-template <typename T, bool NOISE, int CPT>
+// DRIVE: coherent drive E(r) exp(-i omega t) at the stage times (reading Q17), E in shared memory.
+template <typename T, bool NOISE, bool DRIVE, int CPT>
 __global__ void __launch_bounds__(RES_NT, 1)
 resident_pair_kernel(const __grid_constant__ ResidentArgs<T> a) {
     namespace cg = cooperative_groups;
@@ -353,7 +354,8 @@ resident_pair_kernel(const __grid_constant__ ResidentArgs<T> a) {
     C* bufB = bufA + (NB + 1);
     C* bufC = bufB + (NB + 1);
     ushort2* nbr = reinterpret_cast<ushort2*>(bufC + (NB + 1));                   // west, east
-    T* Vs = reinterpret_cast<T*>(nbr + NE);
+    T* Vs = reinterpret_cast<T*>((reinterpret_cast<uintptr_t>(nbr + NE) + 15) & ~(uintptr_t)15);      // (an odd cell count: keep T aligned)
+    C* Es = reinterpret_cast<C*>((reinterpret_cast<uintptr_t>(Vs + NE) + 15) & ~(uintptr_t)15);
 
     const int tid = threadIdx.x, nt = blockDim.x;
     const int real = blockIdx.x / ncta;
@@ -392,6 +394,7 @@ resident_pair_kernel(const __grid_constant__ ResidentArgs<T> a) {
             nb.y = (unsigned short)(i < nx - 1 ? b + 1 : (g.bc_x ? NB : b - nx + 1));
             nbr[c] = nb;
             Vs[c] = (a.V && j >= 0) ? a.V[(size_t)j * nx + i] : T(0);
+            if constexpr (DRIVE) Es[c] = j >= 0 ? a.E[(size_t)j * nx + i] : czero;
             if (j >= 0) { psi[q] = psi_g[(size_t)j * nx + i]; bufA[b] = psi[q]; }
         }
     }
@@ -403,7 +406,7 @@ resident_pair_kernel(const __grid_constant__ ResidentArgs<T> a) {
     (void)has_s; (void)has_n;
     cluster.sync();
 
-    auto odd_stage = [&](const C* in, C* out, auto stage_no) {          // stages 1 and 3, on the extended slab
+    auto odd_stage = [&](const C* in, C* out, auto stage_no, const C qd) {          // stages 1 and 3, on the extended slab
         constexpr int s = decltype(stage_no)::value;
         const T a_dt = s == 3 ? k.dt : k.hdt;
         const T w_dt = s == 1 ? k.dt6 : k.dt3;
@@ -419,14 +422,14 @@ resident_pair_kernel(const __grid_constant__ ResidentArgs<T> a) {
                 Diff<T> df;
                 differences<T, false, false>(k, h, df);
                 T Kn;
-                const C K = deriv<T, false, false, false>(k, h.c, df, czero, df, true, T(0), Vs[c], T(0), czero, czero, Kn);
+                const C K = deriv<T, false, false, DRIVE>(k, h.c, df, czero, df, true, T(0), Vs[c], T(0), DRIVE ? Es[c] : czero, qd, Kn);
                 if (own[q]) acc[q] = fma2s(w_dt, K, s == 1 ? psi[q] : acc[q]);
                 out[b] = fma2s(a_dt, K, psi[q]);
             }
         }
         __syncthreads();
     };
-    auto even_stage = [&](const C* in, C* out, C* out_s, C* out_n, auto stage_no, const uint64_t step) {   // stages 2 and 4, on the slab
+    auto even_stage = [&](const C* in, C* out, C* out_s, C* out_n, auto stage_no, const uint64_t step, const C qd) {   // stages 2 and 4, on the slab
         constexpr int s = decltype(stage_no)::value;
 #pragma unroll
         for (int q = 0; q < CPT; ++q) {
@@ -440,7 +443,7 @@ resident_pair_kernel(const __grid_constant__ ResidentArgs<T> a) {
                 Diff<T> df;
                 differences<T, false, false>(k, h, df);
                 T Kn;
-                const C K = deriv<T, false, false, false>(k, h.c, df, czero, df, true, T(0), Vs[c], T(0), czero, czero, Kn);
+                const C K = deriv<T, false, false, DRIVE>(k, h.c, df, czero, df, true, T(0), Vs[c], T(0), DRIVE ? Es[c] : czero, qd, Kn);
                 C y;
                 if (s == 2) {
                     acc[q] = fma2s(k.dt3, K, acc[q]);
@@ -471,10 +474,19 @@ resident_pair_kernel(const __grid_constant__ ResidentArgs<T> a) {
                 if (c < NE && live[q] && !own[q]) psi[q] = bufA[(c / nx + 1) * nx + c % nx];
             }
         }
-        odd_stage(bufA, bufB, std::integral_constant<int, 1>());
-        even_stage(bufB, bufC, sC, nC, std::integral_constant<int, 2>(), step);
-        odd_stage(bufC, bufB, std::integral_constant<int, 3>());
-        even_stage(bufB, bufA, sA, nA, std::integral_constant<int, 4>(), step);
+        C q1 = czero, q23 = czero, q4 = czero;          // (1/hbar) exp(-i omega t_s) at t, t + dt/2, t + dt, phase in double
+        if constexpr (DRIVE) {
+            auto phase = [&](double cs) {
+                double sn, cn;
+                sincos(-k.omega * (((double)step + cs) * k.dt_d), &sn, &cn);
+                return mk<T>(k.ih * (T)cn, k.ih * (T)sn);
+            };
+            q1 = phase(0.0); q23 = phase(0.5); q4 = phase(1.0);
+        }
+        odd_stage(bufA, bufB, std::integral_constant<int, 1>(), q1);
+        even_stage(bufB, bufC, sC, nC, std::integral_constant<int, 2>(), step, q23);
+        odd_stage(bufC, bufB, std::integral_constant<int, 3>(), q23);
+        even_stage(bufB, bufA, sA, nA, std::integral_constant<int, 4>(), step, q4);
     }
 
 #pragma unroll
@@ -491,9 +503,9 @@ resident_pair_kernel(const __grid_constant__ ResidentArgs<T> a) {
     }
 }
 
-size_t resident_pair_smem_bytes(int nx, int rl, int prec64) {
+size_t resident_pair_smem_bytes(int nx, int rl, int prec64, bool drive = true) {
     const size_t rb = prec64 ? 8 : 4, nb = (size_t)(rl + 4) * nx + 1, ne = (size_t)(rl + 2) * nx;
-    return 3 * nb * 2 * rb + ne * sizeof(ushort2) + ne * rb;
+    return 3 * nb * 2 * rb + ne * sizeof(ushort2) + ne * rb + (drive ? ne * 2 * rb : 0) + 48;      // (+ alignment slack)
 }
 
 // The pair kernel applies to the scalar model when the extended slab fits 4 cells per thread.
@@ -504,11 +516,11 @@ bool resident_pair_ok(int nx, int ny, int ncta, int prec64) {
     return resident_pair_smem_bytes(nx, rl, prec64) <= 200 * 1024;
 }
 
-template <typename T, bool NOISE, int CPT>
+template <typename T, bool NOISE, bool DRIVE, int CPT>
 static cudaError_t launch_pair_one(const ResidentArgs<T>& a, int ncta, cudaStream_t st) {
     const int rl = a.geo.ny / ncta, ne = (rl + 2) * a.geo.nx;
-    const size_t smem = resident_pair_smem_bytes(a.geo.nx, rl, sizeof(T) == 8);
-    auto kern = resident_pair_kernel<T, NOISE, CPT>;
+    const size_t smem = resident_pair_smem_bytes(a.geo.nx, rl, sizeof(T) == 8, DRIVE);
+    auto kern = resident_pair_kernel<T, NOISE, DRIVE, CPT>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     if (ncta > 8) {
@@ -533,8 +545,12 @@ static cudaError_t launch_pair_one(const ResidentArgs<T>& a, int ncta, cudaStrea
 template <typename T>
 static cudaError_t launch_pair_t(const ResidentArgs<T>& a, bool noise, int ncta, cudaStream_t st) {
     const int need = ((a.geo.ny / ncta + 2) * a.geo.nx + RES_NT - 1) / RES_NT;
-    if (noise) return need == 1 ? launch_pair_one<T, true, 1>(a, ncta, st) : launch_pair_one<T, true, 4>(a, ncta, st);
-    return need == 1 ? launch_pair_one<T, false, 1>(a, ncta, st) : launch_pair_one<T, false, 4>(a, ncta, st);
+    if (a.E) {
+        if (noise) return need == 1 ? launch_pair_one<T, true, true, 1>(a, ncta, st) : launch_pair_one<T, true, true, 4>(a, ncta, st);
+        return need == 1 ? launch_pair_one<T, false, true, 1>(a, ncta, st) : launch_pair_one<T, false, true, 4>(a, ncta, st);
+    }
+    if (noise) return need == 1 ? launch_pair_one<T, true, false, 1>(a, ncta, st) : launch_pair_one<T, true, false, 4>(a, ncta, st);
+    return need == 1 ? launch_pair_one<T, false, false, 1>(a, ncta, st) : launch_pair_one<T, false, false, 4>(a, ncta, st);
 }
 
 template <typename T>
@@ -542,6 +558,7 @@ static cudaError_t launch_cluster_t(const ResidentArgs<T>& a, bool res, bool noi
     const int ncta = resident_cluster_size(a.geo.nx, a.geo.ny, sizeof(T) == 8, res);
     if (ncta == 0) return cudaErrorInvalidConfiguration;
     if (PHX_RESIDENT_PAIR && !res && resident_pair_ok(a.geo.nx, a.geo.ny, ncta, sizeof(T) == 8)) return launch_pair_t<T>(a, noise, ncta, st);
+    if (a.E) return cudaErrorInvalidConfiguration;          // (a drive: the pair kernel only)
     const int need = (a.geo.nx * (a.geo.ny / ncta) + RES_NT - 1) / RES_NT;
 #define PHX_RESC_CASE(R, NZ)                                                  \
     if (res == R && noise == NZ) {                                            \
@@ -554,6 +571,12 @@ static cudaError_t launch_cluster_t(const ResidentArgs<T>& a, bool res, bool noi
     PHX_RESC_CASE(true, true)
 #undef PHX_RESC_CASE
     return cudaErrorInvalidConfiguration;
+}
+
+// A driven scalar grid can run variant RESIDENT iff the pair kernel applies to it.
+bool resident_drive_ok(int nx, int ny, int prec64) {
+    const int ncta = resident_cluster_size(nx, ny, prec64, false);
+    return PHX_RESIDENT_PAIR && ncta != 0 && resident_pair_ok(nx, ny, ncta, prec64);
 }
 
 cudaError_t launch_resident_cluster_32(const ResidentArgs<float>& a, bool res, bool noise, cudaStream_t st) { return launch_cluster_t<float>(a, res, noise, st); }

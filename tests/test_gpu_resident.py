@@ -120,7 +120,12 @@ def test_grids_that_do_not_fit_are_refused():
     w = wl.cfg2(n=32, ny=32, prec="c32")
     g = make_gpu(w)
     assert g.get_variant() == RESIDENT             # AUTO: a single small grid runs on a cluster (the cluster form)
-    g.set_drive(np.zeros((32, 32), np.complex64))  # a drive: the fused step takes over
+    g.set_drive(np.zeros((32, 32), np.complex64))  # a drive on a scalar grid: the cluster form carries it
+    assert g.get_variant() == RESIDENT
+    g.destroy()
+    g = make_gpu(wl.cfg3(n=32, prec="c32"))
+    assert g.get_variant() == RESIDENT
+    g.set_drive(np.zeros((32, 32), np.complex64))  # a drive on a reservoir grid: the fused step takes over
     assert g.get_variant() == STEP
     g.destroy()
     g = make_gpu(wl.cfg2(n=33, ny=31, prec="c32"))
@@ -150,7 +155,10 @@ def _noisy(w):
     (lambda: wl.cfg5(n=64, batch=3, prec="c32"), (0, 0)),                 # noise: the cell index of the counter is the grid's
     (lambda: wl.cfg5(n=128, batch=2, prec="c32"), (0, 0)),
     (lambda: _noisy(wl.cfg2(n=64, ny=64, prec="c32")), (0, 0)),           # scalar + noise: the two-stages-per-barrier kernel
-    (lambda: _noisy(wl.cfg2(n=40, ny=24, prec="c64")), (1, 1))])
+    (lambda: _noisy(wl.cfg2(n=40, ny=24, prec="c64")), (1, 1)),
+    (lambda: wl.cfg2(n=33, ny=6, prec="c64"), (0, 0)),                    # an odd number of cells per slab in fp64
+    (lambda: wl.cfg2(n=35, ny=10, prec="c64"), (0, 1)),
+    (lambda: wl.cfg3(n=34, prec="c64"), (0, 0))])
 def test_cluster_form(maker, bc):
     w = maker()
     g = make_gpu(w, variant=RESIDENT, bc=bc, tuning={"resident_cluster": 1})
@@ -190,3 +198,30 @@ def test_cluster_form_opens_resident_to_128_wide_grids():
     with pytest.raises(phx.PhxError):
         g.select_variant(RESIDENT)                         # without the cluster form the request is refused
     g.destroy()
+
+
+
+@pytest.mark.parametrize("prec,nx,ny,bc,noise", [("c64", 64, 64, (0, 0), False), ("c32", 128, 128, (0, 0), False), ("c32", 50, 24, (1, 0), False),
+                                                  ("c64", 33, 6, (0, 1), False), ("c32", 64, 32, (0, 0), True)])
+def test_cluster_form_with_coherent_drive(prec, nx, ny, bc, noise):
+    """E(r) exp(-i omega t) at the stage times (reading Q17) in the cluster form of the scalar
+    model (resident_pair_kernel): against the oracle, and against the fused step to a tenth of the tolerance; AUTO keeps a driven single small scalar grid in RESIDENT."""
+    w = wl.cfg2(n=nx, ny=ny, prec=prec)
+    if noise:
+        w = _noisy(w)
+    rng = np.random.default_rng(31)
+    E = (0.05 * (rng.standard_normal((ny, nx)) + 1j * rng.standard_normal((ny, nx)))).astype(np.complex64 if prec == "c32" else np.complex128)
+    xp = dict(omega=3.7)
+    g = make_gpu(w, bc=bc, E=E, extra_params=xp)
+    assert g.get_variant() == RESIDENT
+    o = make_oracle(w, bc=bc, E=E, extra_params=xp)
+    g.step_rk4(40)
+    g.step_rk4(21)              # (the phase follows the step counter across calls)
+    o.step_rk4(61)
+    compare(g, o, w)
+    ref = make_gpu(w, bc=bc, E=E, extra_params=xp, variant=STEP)
+    ref.step_rk4(61)
+    # (the fused step evaluates the isotropic, hbar = 1 form of the same derivative: rounding-level differences)
+    assert rel_l2(g.read_field("psi_p"), ref.read_field("psi_p")) <= 0.1 * TOL[prec]
+    g.destroy()
+    ref.destroy()
